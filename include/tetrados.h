@@ -1,0 +1,143 @@
+/*
+ * tetrados.h -- C ABI of libtetrados: linear-tetrahedron density of states on one B200.
+ *
+ * The library computes, for band energies E_n(k) and orbital weights
+ * b_{n,m}(k) = |a_n^m(k)|^2 given on a periodic N1 x N2 x N3 k-grid,
+ *
+ *     DOS_m(w) = (1/V_G) sum_n int d^3k b_{n,m}(k) delta(w - E_n(k))      PAPER.md Eq. 4  (:52)
+ *     N_m(w)   = (1/V_G) sum_n int d^3k b_{n,m}(k) Theta(w - E_n(k))      PAPER.md Eq. 2-3 (:43-48)
+ *
+ * by the linear tetrahedron method of arxiv 1710.10789: every cube of the grid is split into
+ * the six tetrahedra of Table I, the four corner energies of each
+ * (tetrahedron, band) are sorted, the corner weights w_l(w) and dw_l/dw of
+ * Eq. 11-15 are evaluated and contracted with the corner orbital weights
+ * (Eq. 8, :91) and summed over tetrahedra and bands (Eq. 9, :96).  Everything runs in CUDA
+ * kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions (part of the ABI)
+ *   k-point index   ik = ix + N1*(iy + N2*iz), ix fastest; k = (ix/N1, iy/N2, iz/N3) in units of the
+ *                   reciprocal lattice vectors; the grid is periodic (index N_d wraps to 0), so there
+ *                   are N1*N2*N3 cubes.  The cube at ik has its corner 1 there; corner label c=1..8 of
+ *                   Table I sits at offset (dx,dy,dz) = bits 0,1,2 of (c-1)   (reading G7).
+ *   normalisation   V_T/V_G = 1/(6 N1 N2 N3); no spin factor.  N_m(w -> inf) = (1/nk) sum_k sum_n b.
+ *   intervals       half-open, tested in the order  w <= E1, w < E2, w < E3, w < E4, else  (reading G10).
+ *   precision       fp32 inputs, fp32 arithmetic for the weights, block-local fp32
+ *                   partial sums, fp64 merge across blocks and fp64 prefix sum for N; fp32 outputs.
+ *   NaN/Inf in E or W are not detected: results are then undefined.
+ *
+ * Ownership: the caller owns every array; the library never frees them and does not retain them
+ * past the call (device mode: past completion of the work queued on `stream`).  A plan owns all
+ * scratch (block partials, staging buffers, its side stream).  A plan must not be used from two
+ * host threads or two streams at the same time.  Inputs are never written.
+ *
+ * Errors: every function returns 0 (TDOS_OK) or a negative code; nothing throws, exits or prints.
+ * On error the outputs are untouched (host mode) / unspecified only if TDOS_ECUDA occurred mid-flight.
+ */
+#ifndef TETRADOS_H
+#define TETRADOS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TDOS_OK       0
+#define TDOS_EINVAL  -1   /* bad argument: NULL where not allowed, N_d < 1, nb/norb/nE < 1, nE > nE_max,
+                             nE > TDOS_MAX_NE, omega not strictly increasing, W == NULL with norb != 1,
+                             bad layout / memspace / slab range                                       */
+#define TDOS_ENOMEM  -2   /* host or device allocation failed                                          */
+#define TDOS_ECUDA   -3   /* a CUDA call failed; see tdos_last_cuda_error()                            */
+#define TDOS_EARCH   -4   /* the selected device is not compute capability 10.x (sm_100)               */
+
+#define TDOS_AOS 0        /* E[ik][n],  W[ik][n][m]   -- what a CPU code usually holds                  */
+#define TDOS_SOA 1        /* E[n][ik],  W[n][m][ik]   -- k fastest                                      */
+
+#define TDOS_DEVICE 0     /* E, W, omega, dos, nos are device pointers (on the plan's device)           */
+#define TDOS_HOST   1     /* they are host pointers (pinned recommended); H2D / D2H done by the library */
+
+#define TDOS_MAX_NE 65534 /* energies per call (bin indices are kept in 16 bits inside the kernel)      */
+
+typedef struct tdos_plan tdos_plan;   /* opaque */
+
+/* Library version (major*100 + minor). */
+int tdos_version(void);
+
+/* Static, never-freed description of an error code. */
+const char* tdos_strerror(int code);
+
+/* Text of the last CUDA error seen by the calling thread ("" if none).  Valid until the next
+ * failing call on this thread. */
+const char* tdos_last_cuda_error(void);
+
+/*
+ * Create a plan for grids of nk[0] x nk[1] x nk[2] k-points, nb bands, norb orbitals and up to
+ * nE_max energies on CUDA device `device`.  Allocates all device scratch:
+ * per-block partial histograms (3 * norb * nE_max floats per resident block) and the fp64 merge
+ * buffers.  *out is set only on success.
+ */
+int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int norb, int nE_max);
+
+/* Free a plan and everything it owns.  NULL is a no-op.  Synchronises the plan's streams first. */
+int tdos_plan_destroy(tdos_plan* p);
+
+/*
+ * The hot path: DOS_m(omega_i) and N_m(omega_i) for all orbitals m and all nE energies.
+ *
+ *  E       band energies, nk*nb floats in `layout`
+ *  W       orbital weights |a_n^m(k)|^2, nk*nb*norb floats in `layout`;
+ *          NULL means W == 1 and requires norb == 1 (total DOS, X = 1)
+ *  omega   nE strictly increasing energies.  A (nearly) uniform grid is located by direct
+ *          index computation plus an exact fix-up; any other increasing grid is still handled
+ *          exactly, only slower.
+ *  dos     out [norb][nE], overwritten
+ *  nos     out [norb][nE], overwritten; may be NULL
+ *  memspace TDOS_DEVICE: all five pointers are device pointers; the call only enqueues work on
+ *          `cuda_stream` (a cudaStream_t, NULL = legacy default stream) and returns.
+ *          TDOS_HOST: all five are host pointers; inputs are staged to the device in z-slabs on the
+ *          plan's side stream, overlapped with the kernels, and the call returns after the results
+ *          are in `dos` / `nos` (`cuda_stream` is ignored).
+ */
+int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+              float* dos, float* nos, int memspace, void* cuda_stream);
+
+/*
+ * Multi-GPU building blocks (device pointers only).
+ * tetra_dos_partial: the additive share of the cubes with z_lo <= iz < z_hi, as raw fp64 sums
+ *   part[3][norb][nE]  (0: sum b*dw/V, 1: in-window sum b*w/V, 2: Eq.-15 step histogram / V),
+ *   overwritten.  E and W must hold the whole grid (the kernel reads planes z_lo .. z_hi, wrapping).
+ * tetra_dos_finalize: dos = V*part[0]; nos = V*(part[1] + inclusive prefix sum over omega of part[2]).
+ * A sum of the `part` arrays of disjoint slabs covering 0..N3 (e.g. an all-reduce) followed by
+ * tetra_dos_finalize equals tetra_dos.
+ */
+int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, const float* omega,
+                      int nE, int z_lo, int z_hi, double* part, void* cuda_stream);
+int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos,
+                       void* cuda_stream);
+
+/*
+ * One-shot convenience matching the paper's "called from a CPU code" scenario:
+ * host pointers, AoS layout, cubic Nk^3 grid, omega_i = (float)(omega_min + i*(omega_max-omega_min)/(nE-1))
+ * evaluated in double (endpoints inclusive).  Creates a plan on the current device,
+ * runs, destroys it.
+ */
+int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, float omega_min,
+                     float omega_max, int nE, float* dos, float* nos);
+
+/*
+ * Diagnostics used by bench.py (not part of the hot path).
+ * tdos_plan_info: what[0] = resident blocks of the main kernel, [1] = threads per block,
+ *   [2] = dynamic shared memory per block (bytes), [3] = work items of the last call,
+ *   [4] = kernel launches of the last tetra_dos / tetra_dos_partial+finalize call,
+ *   [5..7] = tile extent in cubes (x, y, z).
+ * tdos_last_kernel_ms: device time of the main kernel and of the merge+finalize kernels of the
+ *   last call, measured with CUDA events on the call's stream (synchronises that stream).
+ * tdos_fp32_fma_probe: runs a register-resident FFMA chain on every SM of the plan's device and
+ *   returns the achieved FP32 rate in TFLOP/s (2 flops per FMA lane) in *tflops.
+ */
+int tdos_plan_info(const tdos_plan* p, long long what[8]);
+int tdos_last_kernel_ms(tdos_plan* p, float* main_ms, float* merge_ms);
+int tdos_fp32_fma_probe(tdos_plan* p, int packed, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TETRADOS_H */

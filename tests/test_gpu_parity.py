@@ -1,0 +1,176 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by
+element, same seeded inputs.  Tolerances: tests/gpu_util.py (north star)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1710_10789_b200 import binding, workloads as wl
+from gpu_util import run_gpu, assert_parity, errors
+
+pytestmark = pytest.mark.gpu
+
+NT = None
+
+
+def _threads():
+    return oracle.max_threads()
+
+
+def test_cfg1_cosine_band():
+    """BASELINE config 1: closed-form band, Nk=16, W == 1 (W=NULL), 201 energies."""
+    E, W, om = wl.make_inputs("cfg1")
+    ref = oracle.tetra_dos(E, None, (16, 16, 16), om)
+    dos, nos = run_gpu(E, None, (16, 16, 16), om)
+    d, en = assert_parity(ref, dos, nos, "cfg1")
+    print("cfg1 dDOS %.2e dN %.2e" % (d, en))
+    # W given explicitly as ones: same result bit for bit
+    dos2, nos2 = run_gpu(E, W, (16, 16, 16), om)
+    assert np.array_equal(dos, dos2) and np.array_equal(nos, nos2)
+
+
+def test_cfg2_tb8_nk32(cache_dir):
+    """BASELINE config 2: 8-orbital model, Nk=32, 1000 energies; full element-wise comparison."""
+    E, W, om = wl.make_inputs("cfg2", cache_dir)
+    ref = oracle.tetra_dos(E, W, (32, 32, 32), om, windowed=True, nthreads=_threads())
+    dos, nos = run_gpu(E, W, (32, 32, 32), om)
+    d, en = assert_parity(ref, dos, nos, "cfg2")
+    print("cfg2 dDOS %.2e dN %.2e" % (d, en))
+
+
+@pytest.mark.parametrize("nk,nb,norb,nE", [
+    ((2, 2, 2), 1, 1, 17),        # minimal periodic grid: every neighbour is a wrap
+    ((1, 1, 1), 2, 3, 9),         # a single k-point: all four corners degenerate
+    ((5, 3, 7), 3, 5, 333),       # anisotropic, ragged against every tile shape, norb not a power of 2
+    ((9, 10, 11), 2, 8, 1000),
+    ((17, 8, 5), 1, 2, 64),
+    ((6, 6, 6), 4, 12, 257),      # norb > 8: two orbital blocks
+    ((4, 4, 4), 2, 4, 1),         # a single energy
+])
+def test_random_small_grids(nk, nb, norb, nE):
+    E, W = wl.random_bands(nk, nb, norb, seed=100 + nk[0] + nE)
+    om = wl.omega_grid(-1.2, 1.3, nE)
+    ref = oracle.tetra_dos(E, W, nk, om)
+    for layout in (binding.TDOS_AOS, binding.TDOS_SOA):
+        Ex, Wx = (E, W) if layout == binding.TDOS_AOS else wl.to_soa(E, W)
+        dos, nos = run_gpu(Ex, Wx, nk, om, layout=layout)
+        assert_parity(ref, dos, nos, "random %s layout %d" % (nk, layout))
+    dos, nos = run_gpu(E, W, nk, om, memspace=binding.TDOS_HOST)
+    assert_parity(ref, dos, nos, "random %s host" % (nk,))
+    dos, nos = run_gpu(E, W, nk, om, want_nos=False)
+    assert nos is None
+    assert_parity(ref, dos, None, "random %s nos=NULL" % (nk,))
+
+
+def test_ties_and_energies_on_corner_values():
+    """Energies on a coarse lattice (many exact ties, flat tetrahedra) and omega exactly ON corner
+    energies: the half-open interval rules (G10) decide; results must match the oracle."""
+    nk, nb, norb = (6, 5, 4), 3, 3
+    rng = np.random.default_rng(7)
+    n = int(np.prod(nk))
+    E = np.sort(rng.integers(-8, 9, (n, nb)) / 8.0, axis=1).astype(np.float32)
+    W = rng.uniform(0, 1, (n, nb, norb)).astype(np.float32)
+    om = (np.arange(-20, 21) / 16.0).astype(np.float32)       # every second point hits lattice values
+    ref = oracle.tetra_dos(E, W, nk, om)
+    dos, nos = run_gpu(E, W, nk, om)
+    assert_parity(ref, dos, nos, "ties")
+
+
+def test_flat_band_and_grid_outside_bands():
+    nk = (4, 4, 4)
+    E = np.full((64, 1), 0.25, dtype=np.float32)
+    W = np.full((64, 1, 2), 0.5, dtype=np.float32)
+    om = np.array([0.0, 0.25, 0.5, 0.75], dtype=np.float32)
+    dos, nos = run_gpu(E, W, nk, om)
+    assert not dos.any()
+    assert np.allclose(nos, [[0, 0, 0.5, 0.5]] * 2, atol=1e-7)
+    E, W = wl.random_bands(nk, 2, 2, seed=3)
+    lo = np.array([-5.0, -4.0], dtype=np.float32)
+    hi = np.array([4.0, 5.0], dtype=np.float32)
+    d, n = run_gpu(E, W, nk, lo)
+    assert not d.any() and not n.any()
+    d, n = run_gpu(E, W, nk, hi)
+    assert not d.any()
+    assert np.allclose(n, W.astype(np.float64).sum(axis=(0, 1))[:, None] / 64, rtol=1e-6)
+
+
+def test_nonuniform_omega_grid():
+    """Any strictly increasing grid is handled exactly (index guess + exact fix-up)."""
+    nk, nb, norb = (7, 7, 7), 2, 2
+    E, W = wl.random_bands(nk, nb, norb, seed=21)
+    rng = np.random.default_rng(1)
+    om = np.unique(np.concatenate([np.linspace(-1.5, -0.5, 10), np.sort(rng.uniform(-0.5, 0.6, 150)),
+                                   np.linspace(0.6, 1.5, 7)]).astype(np.float32))
+    ref = oracle.tetra_dos(E, W, nk, om)
+    dos, nos = run_gpu(E, W, nk, om)
+    assert_parity(ref, dos, nos, "nonuniform")
+
+
+def test_partial_slabs_and_finalize():
+    """tetra_dos_partial over disjoint z-slabs, summed, then tetra_dos_finalize == tetra_dos
+    (the multi-GPU building blocks), and each slab's share matches the oracle's cube range."""
+    import torch
+    nk, nb, norb, nE = (6, 5, 9), 2, 3, 200
+    E, W = wl.random_bands(nk, nb, norb, seed=5)
+    om = wl.omega_grid(-1.2, 1.3, nE)
+    ref = oracle.tetra_dos(E, W, nk, om)
+    dev = torch.device("cuda:0")
+    dE, dW, dOm = (torch.from_numpy(x).to(dev) for x in (E, W, om))
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        total = torch.zeros((3, norb, nE), dtype=torch.float64, device=dev)
+        for z_lo, z_hi in ((0, 4), (4, 5), (5, 9)):
+            part = torch.empty((3, norb, nE), dtype=torch.float64, device=dev)
+            plan.tetra_dos_partial(dE, dW, dOm, z_lo, z_hi, part)
+            total += part
+        dos = torch.empty((norb, nE), device=dev)
+        nos = torch.empty((norb, nE), device=dev)
+        plan.tetra_dos_finalize(total, nE, dos, nos)
+        torch.cuda.synchronize()
+        assert_parity(ref, dos.cpu().numpy(), nos.cpu().numpy(), "slabs")
+        # one slab against the oracle's share of the same cubes
+        part = torch.empty((3, norb, nE), dtype=torch.float64, device=dev)
+        plan.tetra_dos_partial(dE, dW, dOm, 4, 5, part)
+        plan.tetra_dos_finalize(part, nE, dos, nos)
+        torch.cuda.synchronize()
+        sl = oracle.tetra_dos(E, W, nk, om, cube_range=(4 * 30, 5 * 30))
+        d = np.abs(dos.cpu().numpy() - sl["dos"]).max() / ref["dos"].max()
+        n = np.abs(nos.cpu().numpy() - sl["nos"]).max() / ref["nos"].max()
+        assert d < 1e-5 and n < 1e-6
+
+
+def test_error_codes_on_gpu():
+    import torch
+    nk, nb, norb, nE = (4, 4, 4), 1, 2, 16
+    E, W = wl.random_bands(nk, nb, norb, seed=1)
+    om = wl.omega_grid(-1, 1, nE)
+    dev = torch.device("cuda:0")
+    dE, dW, dOm = (torch.from_numpy(x).to(dev) for x in (E, W, om))
+    dos = torch.zeros((norb, nE), device=dev)
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        with pytest.raises(binding.TdosError) as ei:   # W == NULL needs norb == 1
+            plan.tetra_dos(dE, None, dOm, dos)
+        assert ei.value.code == binding.TDOS_EINVAL
+        with pytest.raises(binding.TdosError):         # nE > nE_max
+            plan.tetra_dos(dE, dW, torch.zeros(nE + 1, device=dev), dos)
+        with pytest.raises(binding.TdosError):         # bad layout
+            plan.tetra_dos(dE, dW, dOm, dos, layout=7)
+        with pytest.raises(binding.TdosError):         # host mode validates omega
+            bad = om.copy()
+            bad[3] = bad[2]
+            plan.tetra_dos(E, W, bad, np.zeros((norb, nE), dtype=np.float32), memspace=binding.TDOS_HOST)
+        with pytest.raises(binding.TdosError):         # bad slab
+            plan.tetra_dos_partial(dE, dW, dOm, 3, 9, torch.zeros((3, norb, nE), dtype=torch.float64, device=dev))
+        assert not dos.any()                           # outputs untouched on error
+        plan.tetra_dos(dE, dW, dOm, dos)               # and the plan is still usable
+        torch.cuda.synchronize()
+        assert dos.any()
+
+
+def test_tetra_dos_simple_host_oneshot():
+    E, W = wl.tb8_bands((10, 10, 10), threads=1)
+    nE = 300
+    om = wl.omega_grid(-6.0, 4.0, nE)
+    ref = oracle.tetra_dos(E, W, (10, 10, 10), om, nthreads=_threads())
+    dos = np.zeros((8, nE), dtype=np.float32)
+    nos = np.zeros((8, nE), dtype=np.float32)
+    binding.tetra_dos_simple(E, W, 10, 8, 8, -6.0, 4.0, nE, dos, nos)
+    assert_parity(ref, dos, nos, "simple")
