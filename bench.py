@@ -1,0 +1,357 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the tetrahedron-DOS hot path (arxiv 1710.10789) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (implicit cube/tetrahedron indexing,
+corner sort, energy window, corner weights Eq. 11-15, orbital projection, accumulation, fp64 merge +
+prefix sum) over one synthetic workload -- by default BASELINE.json configs[3] (the headline roofline
+config: seeded 8-orbital model, Nk=128, 4000 energies), inputs already resident in HBM.
+
+Prints ONE JSON line (rank 0).  `value` = nominal (tetrahedron, band, omega) evaluations per second,
+n_tb*nE / t, the paper's accounting (every energy of every (tetrahedron, band));
+`effective_evals_per_s` counts only the n_eval evaluations with E1 < omega < E4 the method needs.
+`roofline` is the main kernel against the FP32-ALU peak; `e2e` is the same
+metric through the C-ABI call with HOST buffers (H2D + kernels + D2H inside the timed region);
+`cpu_baseline` is the fp64 oracle on this box's host cores on a bounded sample of the same workload.
+
+--impl reference times the oracle (the only "reference" this paper-only tier has) on the same config,
+each step a bounded sample.  N > 1 (torchrun): the cubes are sharded in z-slabs, one rank per GPU,
+each rank's additive fp64 partial is all-reduced (NCCL) and finalised -- strong scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1710_10789_b200 import workloads as wl  # noqa: E402  (input generators only)
+
+# Algorithmic flop model: per in-window evaluation
+# F_eval = 40 + 18*norb (weights of Eq. 12-14 case-averaged + 2*4*norb FMAs + 2*norb adds), per
+# (tetrahedron, band) F_tb = 40 + 5*norb (sort, differences, reciprocals, Eq.-15 sum).
+def flops_alg(n_eval: int, n_tb: int, norb: int) -> float:
+    return float(n_eval) * (40 + 18 * norb) + float(n_tb) * (40 + 5 * norb)
+
+
+# FP32-ALU peak derived from the guide's unit counts and clocks: SMs x 128 FP32 lanes x 2 flops (FMA)
+# x max SM clock (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz).
+def fp32_peak_tflops(num_sms: int, sm_max_mhz: float) -> float:
+    return num_sms * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg4", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cache", default=os.environ.get("TDOS_CACHE", "/tmp/tdos_cache"))
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self.period = period_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------------------------
+# The oracle legs (the ONLY places bench.py touches oracle/): cpu_baseline and --impl reference.
+# ----------------------------------------------------------------------------------------------
+def oracle_sample_planes(cfg) -> int:
+    """Bounded sample of the workload: the cubes of the first N3/16 z-planes (>= 1)."""
+    return max(1, cfg.nk[2] // 16)
+
+
+def run_oracle_sample(cfg, E, W, om, reps: int = 1, warmup: int = 0):
+    """Time the fp64 oracle, as it stands, on the sample.  Returns (seconds per rep, n_tb, n_eval, cores, text)."""
+    import oracle
+    oracle.build()
+    planes = oracle_sample_planes(cfg)
+    hi = cfg.nk[0] * cfg.nk[1] * planes
+    cores = min(oracle.max_threads(), len(os.sched_getaffinity(0)))
+    Wn = None if cfg.model == "cosine" else W
+    times, res = [], None
+    for r in range(warmup + reps):
+        t0 = time.perf_counter()
+        res = oracle.tetra_dos(E, Wn, cfg.nk, om, windowed=True, nthreads=cores, cube_range=(0, hi))
+        if r >= warmup:
+            times.append(time.perf_counter() - t0)
+    text = ("oracle.tetra_dos(windowed=True: Eq. 12-14 inside (E1,E4), Eq. 15 by step+prefix), fp64, OpenMP over cubes, "
+            "on the cubes of z-planes [0,%d) of %s (%d of %d cubes), all %d energies"
+            % (planes, cfg.name, hi, int(np.prod(cfg.nk)), cfg.nE))
+    return float(np.mean(times)), res["n_tb"], res["n_eval"], cores, text
+
+
+def reference_arm(args, cfg, rank: int):
+    """--impl reference: the oracle on host cores, rank 0 only."""
+    if rank != 0:
+        return
+    E, W, om = wl.make_inputs(cfg, args.cache)
+    sec, n_tb, n_eval, cores, text = run_oracle_sample(cfg, E, W, om, reps=args.steps, warmup=args.warmup)
+    value = n_tb * cfg.nE / sec
+    line = {
+        "impl": "reference", "metric": "tetra*band*omega evaluations/sec", "value": value, "unit": "eval/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, args.gpus),
+        "effective_evals_per_s": n_eval / sec,
+        "cpu_baseline": {"value": value, "unit": "eval/s", "cores": cores, "kind": "oracle", "sample": text},
+        "e2e": {"value": value, "unit": "eval/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, n_gpus: int) -> dict:
+    return {"workload": "%s: %s, Nk=%dx%dx%d, nb=%d, norb=%d, nE=%d on [%g,%g]" % (
+                cfg.name, "seeded 8-orbital tetragonal tight-binding" if cfg.model == "tb8" else "simple-cubic cosine band",
+                cfg.nk[0], cfg.nk[1], cfg.nk[2], cfg.nb, cfg.norb, cfg.nE, cfg.omega_min, cfg.omega_max),
+            "nk": list(cfg.nk), "nb": cfg.nb, "norb": cfg.norb, "nE": cfg.nE, "layout": "AoS E[ik][n], W[ik][n][m]",
+            "parallelism": "1 GPU" if n_gpus == 1 else "z-slabs over %d GPUs + all-reduce of fp64 partials" % n_gpus}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the main kernel, from the committed
+# `ncu --set full` capture (profiles/, named there); None until a capture of that config exists.
+NCU_TRAFFIC_BYTES = {}
+
+
+def main():
+    args = parse_args()
+    cfg = wl.CONFIGS[args.config]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        reference_arm(args, cfg, rank)
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    from paper_1710_10789_b200 import binding   # raises if libtetrados.so is missing: no CPU fallback
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    # ---- inputs (seeded, synthetic; rank 0 diagonalises and caches, the others load the cache)
+    if rank == 0:
+        E, W, om = wl.make_inputs(cfg, args.cache)
+    barrier()
+    if rank != 0:
+        E, W, om = wl.make_inputs(cfg, args.cache)
+    N1, N2, N3 = cfg.nk
+    nb, norb, nE = cfg.nb, cfg.norb, cfg.nE
+    unitW = cfg.model == "cosine"
+    dE = torch.from_numpy(E).to(dev)
+    dW = None if unitW else torch.from_numpy(W).to(dev)
+    dOm = torch.from_numpy(om).to(dev)
+    dos = torch.zeros((norb, nE), device=dev)
+    nos = torch.zeros((norb, nE), device=dev)
+    part = torch.zeros((3, norb, nE), dtype=torch.float64, device=dev)
+    z_lo, z_hi = (N3 * rank) // world, (N3 * (rank + 1)) // world
+    plan = binding.Plan(cfg.nk, nb, norb, nE, device=local_rank)
+
+    def step():
+        if world == 1:
+            plan.tetra_dos(dE, dW, dOm, dos, nos)
+        else:
+            plan.tetra_dos_partial(dE, dW, dOm, z_lo, z_hi, part)
+            dist.all_reduce(part)                      # the path's one exchange step
+            plan.tetra_dos_finalize(part, nE, dos, nos)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop()
+    ms = torch.tensor([ev0.elapsed_time(ev1) / args.steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_per_step = float(ms.item())
+
+    # ---- work counters (exact integers from the kernel) and per-kernel device times of the timed steps
+    main_ms, merge_ms = plan.kernel_ms(min(args.steps, 64))
+    cnt = plan.last_counters()
+    c = torch.tensor([cnt["n_tb"], cnt["n_eval"]], dtype=torch.int64, device=dev)
+    if world > 1:
+        dist.all_reduce(c)
+        km = torch.tensor([main_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(km, op=dist.ReduceOp.MAX)
+        main_ms = float(km.item())
+    n_tb, n_eval = int(c[0].item()), int(c[1].item())
+    info = plan.info()
+    launches_per_step = 3   # main + merge + finalize (memsets and NCCL not counted)
+
+    # ---- e2e: the same step through the C-ABI with HOST (pinned) buffers
+    e2e = None
+    if not args.no_e2e:
+        hE = torch.from_numpy(E).pin_memory()
+        hW = None if unitW else torch.from_numpy(W).pin_memory()
+        hOm = torch.from_numpy(om).pin_memory()
+        hdos = torch.zeros((norb, nE)).pin_memory()
+        hnos = torch.zeros((norb, nE)).pin_memory()
+        plane = N1 * N2
+
+        def e2e_step():
+            if world == 1:
+                plan.tetra_dos(hE, hW, hOm, hdos, hnos, memspace=binding.TDOS_HOST)
+                return
+            # each rank stages its own z-slab plus the halo plane, then partial -> all-reduce -> finalize
+            a, b = z_lo * plane, z_hi * plane
+            h = (z_hi % N3) * plane
+            dE[a:b].copy_(hE[a:b], non_blocking=True)
+            dE[h:h + plane].copy_(hE[h:h + plane], non_blocking=True)
+            if hW is not None:
+                dW[a:b].copy_(hW[a:b], non_blocking=True)
+                dW[h:h + plane].copy_(hW[h:h + plane], non_blocking=True)
+            dOm.copy_(hOm, non_blocking=True)
+            step()
+            if rank == 0:
+                hdos.copy_(dos, non_blocking=True)
+                hnos.copy_(nos, non_blocking=True)
+            torch.cuda.synchronize()
+
+        for _ in range(2):
+            e2e_step()
+        torch.cuda.synchronize()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        barrier()
+        t = torch.tensor([(time.perf_counter() - t0) / args.e2e_steps], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+        h2d = E.nbytes + (0 if unitW else W.nbytes) + om.nbytes
+        if world > 1:   # halo planes are copied twice across the job
+            h2d += world * plane * 4 * nb * (1 + (0 if unitW else norb)) + (world - 1) * om.nbytes
+        e2e = {"value": n_tb * nE / e2e_s, "unit": "eval/s", "ms_per_step": e2e_s * 1e3,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(2 * norb * nE * 4),
+               "h2d_gbs": h2d / e2e_s / 1e9}
+
+    # ---- roofline of the dominant kernel (tdos_main): FP32 ALU
+    props = torch.cuda.get_device_properties(dev)
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    peak = fp32_peak_tflops(props.multi_processor_count, sm_max)
+    fl = flops_alg(n_eval, n_tb, norb) / world          # per launch (each rank's share on average)
+    achieved = fl / (main_ms * 1e-3) / 1e12
+    bytes_alg = 4.0 * N1 * N2 * N3 * nb * (1 + (0 if unitW else norb)) + 8.0 * norb * nE
+    roofline = {"bound": "alu", "kernel": "tdos_main", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+                "peak_source": "derived: %d SMs x 128 FP32 lanes x 2 x %.0f MHz (B200_PROFILING.md unit counts and clocks)"
+                               % (props.multi_processor_count, sm_max),
+                "flops_alg_per_launch": fl, "main_kernel_ms": main_ms, "merge_finalize_ms": merge_ms,
+                "bytes_alg": bytes_alg, "hbm_gbs_at_main_kernel": bytes_alg / world / (main_ms * 1e-3) / 1e9}
+    try:
+        roofline["fma_probe_tflops"] = {"ffma": plan.fp32_fma_probe(False), "ffma2": plan.fp32_fma_probe(True)}
+    except Exception as ex:   # diagnostics only
+        roofline["fma_probe_tflops"] = str(ex)
+
+    line = {
+        "metric": "tetra*band*omega evaluations/sec", "value": n_tb * nE / (ms_per_step * 1e-3), "unit": "eval/s",
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": dict(workload_config(cfg, world), l2="inputs (%.0f MB) larger than L2 (126 MB), no flush" % (bytes_alg / 1e6)
+                       if bytes_alg > 126e6 else "inputs fit in L2; L2 not flushed between steps",
+                       tile=list(info["tile"]), grid=info["grid"], threads=info["threads"], smem=info["smem"]),
+        "effective_evals_per_s": n_eval / (ms_per_step * 1e-3), "dos_grids_per_s": 1e3 / ms_per_step,
+        "n_tb": n_tb, "n_eval": n_eval,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
+    }
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sec, s_tb, s_eval, cores, text = run_oracle_sample(cfg, E, W, om)
+        line["cpu_baseline"] = {"value": s_tb * nE / sec, "unit": "eval/s", "cores": cores, "kind": "oracle",
+                                "sample": text, "seconds": sec, "effective_evals_per_s": s_eval / sec}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -18,7 +18,7 @@ TDOS_MAX_NE = 65534
 # every symbol include/tetrados.h declares
 SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy",
            "tetra_dos", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
-           "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
+           "tdos_last_counters", "tdos_kernel_ms", "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
 
 _lib = None
 
@@ -54,6 +54,8 @@ def load():
     lib.tetra_dos_finalize.argtypes = [vp, vp, C.c_int, fp, fp, vp]
     lib.tetra_dos_simple.argtypes = [fp, fp, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_int, fp, fp]
     lib.tdos_plan_info.argtypes = [vp, C.POINTER(C.c_longlong)]
+    lib.tdos_last_counters.argtypes = [vp, C.POINTER(C.c_longlong)]
+    lib.tdos_kernel_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     lib.tdos_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     lib.tdos_fp32_fma_probe.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     for name in SYMBOLS:
@@ -129,10 +131,19 @@ class Plan:
         _check(load().tdos_plan_info(self._h, w), "tdos_plan_info")
         return {"grid": w[0], "threads": w[1], "smem": w[2], "items": w[3], "launches": w[4], "tile": (w[5], w[6], w[7])}
 
-    def last_kernel_ms(self):
+    def last_counters(self) -> dict:
+        w = (C.c_longlong * 2)()
+        _check(load().tdos_last_counters(self._h, w), "tdos_last_counters")
+        return {"n_tb": w[0], "n_eval": w[1]}
+
+    def kernel_ms(self, ncalls: int = 1):
+        """(main kernel ms, merge+finalize ms), mean over the last `ncalls` device-mode calls."""
         a, b = C.c_float(), C.c_float()
-        _check(load().tdos_last_kernel_ms(self._h, C.byref(a), C.byref(b)), "tdos_last_kernel_ms")
+        _check(load().tdos_kernel_ms(self._h, int(ncalls), C.byref(a), C.byref(b)), "tdos_kernel_ms")
         return a.value, b.value
+
+    def last_kernel_ms(self):
+        return self.kernel_ms(1)
 
     def fp32_fma_probe(self, packed: bool = False) -> float:
         t = C.c_double()

@@ -41,6 +41,7 @@ struct MainParams {
     int n_items;                 // ntx*nty*ntz*nb*nmb
     int unitW;                   // W == 1
     float* partial;              // [gridDim.x][3][norb][nE]
+    unsigned long long* counters;   // [0] n_tb, [1] n_eval = #(tb, omega) with E1 < omega < E4
 };
 
 // Table I of the paper, corner labels 1..8 -> 0..7; label c sits at offset
@@ -163,6 +164,7 @@ __global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
         // ---- A2/A3: one thread per (tetrahedron, band): sort, window, record
         {
             int lmin = 0x7fffffff, lmax = -1;
+            unsigned cnt_tb = 0, cnt_ev = 0;
             for (int t = tid; t < NTB; t += NT) {
                 const int tet = t / NC, cube = t - tet * NC;
                 const int cx = cube % TX, cy = (cube / TX) % TY, cz = cube / (TX * TY);
@@ -187,6 +189,8 @@ __global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
                     const int i1 = locate_bin<true>(omega, nE, om0, inv_dom, e0);      // first omega > E1
                     const int i4 = (e3 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e3) : i1;   // first omega >= E4 (and > E1)
                     rng = (uint32_t)i1 | ((uint32_t)i4 << 16);
+                    cnt_tb += 1;
+                    cnt_ev += (unsigned)(i4 - i1);
                     if (i1 < nE) {
                         lmin = min(lmin, i1);
                         lmax = max(lmax, min(i4, nE - 1));
@@ -201,6 +205,14 @@ __global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
             if (lane == 0 && lmax >= 0) {
                 atomicMin(&sMinMax[0], lmin);
                 atomicMax(&sMinMax[1], lmax);
+            }
+            if (mb == 0) {   // work counters (exact integers; bench.py's flop count uses them)
+                cnt_tb = __reduce_add_sync(0xffffffffu, cnt_tb);
+                cnt_ev = __reduce_add_sync(0xffffffffu, cnt_ev);
+                if (lane == 0) {
+                    atomicAdd(p.counters + 0, (unsigned long long)cnt_tb);
+                    atomicAdd(p.counters + 1, (unsigned long long)cnt_ev);
+                }
             }
         }
         __syncthreads();

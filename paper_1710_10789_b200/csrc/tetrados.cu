@@ -74,6 +74,7 @@ struct tdos_plan {
     int grid = 0;
     float* partial = nullptr;     // [grid][3][norb][nE_max]
     double* part64 = nullptr;     // [3][norb][nE_max]
+    unsigned long long* counters = nullptr;   // [2] n_tb, n_eval of the last call
     // host-mode staging
     float* dE = nullptr;
     float* dW = nullptr;
@@ -82,8 +83,14 @@ struct tdos_plan {
     float* dNos = nullptr;
     cudaStream_t side = nullptr;
     cudaStream_t main = nullptr;
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // [3] and [2] bracket the FMA probe
+    // ring of event triples (before main kernel, after it, after merge+finalize), one per tetra_dos call
+    static constexpr int kRing = 64;
+    cudaEvent_t ring[kRing][3] = {};
+    long long n_timed_calls = 0;   // tetra_dos (device path) calls since plan creation
+    int cur_slot = 0;
     cudaStream_t last_stream = nullptr;
+    bool last_stream_valid = false;
     bool timed = false;
     long long last_items = 0, last_launches = 0;
 };
@@ -112,6 +119,7 @@ int tdos_plan_destroy(tdos_plan* p) {
     if (p->main) cudaStreamSynchronize(p->main);
     cudaFree(p->partial);
     cudaFree(p->part64);
+    cudaFree(p->counters);
     cudaFree(p->dE);
     cudaFree(p->dW);
     cudaFree(p->dOm);
@@ -119,6 +127,9 @@ int tdos_plan_destroy(tdos_plan* p) {
     cudaFree(p->dNos);
     for (auto& e : p->ev)
         if (e) cudaEventDestroy(e);
+    for (auto& tr : p->ring)
+        for (auto& e : tr)
+            if (e) cudaEventDestroy(e);
     if (p->side) cudaStreamDestroy(p->side);
     if (p->main) cudaStreamDestroy(p->main);
     delete p;
@@ -165,7 +176,8 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
 
     const size_t hist = (size_t)3 * norb * nE_max;
     if (cudaMalloc(&p->partial, hist * p->grid * sizeof(float)) != cudaSuccess ||
-        cudaMalloc(&p->part64, hist * sizeof(double)) != cudaSuccess) {
+        cudaMalloc(&p->part64, hist * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&p->counters, 2 * sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError();
         tdos_plan_destroy(p);
         return TDOS_ENOMEM;
@@ -182,6 +194,13 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
             tdos_plan_destroy(p);
             return rc;
         }
+    for (auto& tr : p->ring)
+        for (auto& ev : tr)
+            if (cudaEventCreate(&ev) != cudaSuccess) {
+                int rc = cuda_fail(cudaGetLastError(), "cudaEventCreate");
+                tdos_plan_destroy(p);
+                return rc;
+            }
     *out = p;
     return TDOS_OK;
 }
@@ -222,20 +241,23 @@ static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int lay
     mp.n_items = (int)items;
     mp.unitW = (W == nullptr);
     mp.partial = p->partial;
+    mp.counters = p->counters;
 
     const size_t hist = (size_t)3 * p->norb * nE;
     const int grid = (int)((items < p->grid) ? (items > 0 ? items : 1) : p->grid);
     CK(cudaMemsetAsync(p->partial, 0, hist * grid * sizeof(float), st));
-    CK(cudaEventRecord(p->ev[0], st));
+    CK(cudaMemsetAsync(p->counters, 0, 2 * sizeof(unsigned long long), st));
+    CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
     v.fn<<<grid, v.NT, v.smem, st>>>(mp);
     CK(cudaGetLastError());
-    CK(cudaEventRecord(p->ev[1], st));
+    CK(cudaEventRecord(p->ring[p->cur_slot][1], st));
     const int mblocks = (int)((hist + 255) / 256);
     tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, grid, hist, part_out);
     CK(cudaGetLastError());
     p->last_items = items;
     p->last_launches = 2;
     p->last_stream = st;
+    p->last_stream_valid = true;
     p->timed = false;
     return TDOS_OK;
 }
@@ -253,7 +275,13 @@ int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, 
     if (rc) return rc;
     if (!part || z_lo < 0 || z_hi > p->nk[2] || z_lo > z_hi) return TDOS_EINVAL;
     CK(cudaSetDevice(p->device));
-    return enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream);
+    p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
+    rc = enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream);
+    if (rc) return rc;
+    CK(cudaEventRecord(p->ring[p->cur_slot][2], (cudaStream_t)cuda_stream));
+    p->n_timed_calls++;
+    p->timed = true;
+    return TDOS_OK;
 }
 
 int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos, void* cuda_stream) {
@@ -264,11 +292,13 @@ int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, flo
 
 static int run_device(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
                       float* dos, float* nos, cudaStream_t st) {
+    p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
     int rc = enqueue_partial(p, E, W, layout, omega, nE, 0, p->nk[2], p->part64, st);
     if (rc) return rc;
     rc = enqueue_finalize(p, p->part64, nE, dos, nos, st);
     if (rc) return rc;
-    CK(cudaEventRecord(p->ev[2], st));
+    CK(cudaEventRecord(p->ring[p->cur_slot][2], st));
+    p->n_timed_calls++;
     p->last_launches = 3;
     p->timed = true;
     return TDOS_OK;
@@ -348,14 +378,38 @@ int tdos_plan_info(const tdos_plan* p, long long what[8]) {
     return TDOS_OK;
 }
 
-int tdos_last_kernel_ms(tdos_plan* p, float* main_ms, float* merge_ms) {
-    if (!p || !main_ms || !merge_ms || !p->timed) return TDOS_EINVAL;
+int tdos_last_counters(tdos_plan* p, long long cnt[2]) {
+    if (!p || !cnt || !p->last_stream_valid) return TDOS_EINVAL;
     CK(cudaSetDevice(p->device));
-    CK(cudaEventSynchronize(p->ev[2]));
-    CK(cudaEventElapsedTime(main_ms, p->ev[0], p->ev[1]));
-    CK(cudaEventElapsedTime(merge_ms, p->ev[1], p->ev[2]));
+    CK(cudaStreamSynchronize(p->last_stream));
+    unsigned long long h[2];
+    CK(cudaMemcpy(h, p->counters, sizeof(h), cudaMemcpyDeviceToHost));
+    cnt[0] = (long long)h[0];
+    cnt[1] = (long long)h[1];
     return TDOS_OK;
 }
+
+int tdos_kernel_ms(tdos_plan* p, int ncalls, float* main_ms, float* merge_ms) {
+    if (!p || !main_ms || !merge_ms || !p->timed || ncalls < 1 || ncalls > tdos_plan::kRing ||
+        ncalls > p->n_timed_calls)
+        return TDOS_EINVAL;
+    CK(cudaSetDevice(p->device));
+    double a = 0.0, b = 0.0;
+    for (int j = 0; j < ncalls; j++) {
+        cudaEvent_t* tr = p->ring[(p->n_timed_calls - 1 - j) % tdos_plan::kRing];
+        CK(cudaEventSynchronize(tr[2]));
+        float x = 0.f, y = 0.f;
+        CK(cudaEventElapsedTime(&x, tr[0], tr[1]));
+        CK(cudaEventElapsedTime(&y, tr[1], tr[2]));
+        a += x;
+        b += y;
+    }
+    *main_ms = (float)(a / ncalls);
+    *merge_ms = (float)(b / ncalls);
+    return TDOS_OK;
+}
+
+int tdos_last_kernel_ms(tdos_plan* p, float* main_ms, float* merge_ms) { return tdos_kernel_ms(p, 1, main_ms, merge_ms); }
 
 int tdos_fp32_fma_probe(tdos_plan* p, int packed, double* tflops) {
     if (!p || !tflops) return TDOS_EINVAL;
