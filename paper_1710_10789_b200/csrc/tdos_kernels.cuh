@@ -1,23 +1,26 @@
 // tdos_kernels.cuh -- sm_100a kernels of the tetrahedron-DOS hot path.
 //
-// Main kernel `tdos_main`: persistent blocks; one work item = (tile of TX x TY x TZ cubes, band n,
-// block of MB orbitals).  Per item:
-//   A1/A2  the tile's (TX+1)(TY+1)(TZ+1) k-points of E (band n) and W (band n, MB orbitals) are
-//          staged once in shared memory with periodic wrap -- tetrahedra are never materialised;
-//          one thread per (tetrahedron, band) sorts its 4 corner energies (5 compare-exchanges
-//          carrying the corner slots) and stores the record {e1..e4, 4 corner slots, bin window}.
+// Main kernel `tdos_main`: one persistent block per SM; every WARP is an autonomous worker with its
+// own slice of shared memory (no block barriers at all).  One work item = (tile of TX x TY x TZ cubes,
+// band n, block of MB orbitals).  Per item, a warp does
+//   A1/A2  stage the tile's (TX+1)(TY+1)(TZ+1) k-points of E (band n) and W (band n, MB orbitals) in
+//          its shared-memory slice, with periodic wrap -- tetrahedra are never materialised; lane =
+//          (tetrahedron, band) record: sort the 4 corner energies (5 compare-exchanges carrying the
+//          corner slots), store {e1..e4, 4 corner slots};
 //   A3     bin window: i1 = first bin with omega > e1, i4 = first bin with omega >= e4 -- exact,
-//          decided on the fp32 omega values themselves.
-//   A4-A6  every thread OWNS one energy bin of the tile's energy span and keeps its 2*MB sums
-//          (DOS and in-window N) in registers: 8 consecutive lanes form a group that walks, on its
-//          own, the records whose window overlaps the group's 8 bins; the record is a shared-memory
-//          broadcast, the lane evaluates Eq. 12/13/14 at its own omega and does the 4 x MB
-//          projection as FMAs into its registers.  No atomics, no write conflicts (the paper's
-//          "thread = energy, thread-local accumulation", restricted to the window).
-//          The Eq.-15 constant of finished tetrahedra goes into a block-local step histogram
-//          (shared memory) at bin i4.
-//   flush  registers + step histogram are added to this block's private partial histogram in HBM
-//          (plain read-modify-write, the block is its only writer).
+//          decided on the fp32 omega values themselves;
+//   A6'    Eq. 15: the constant sum_l b_l of a finished tetrahedron goes, as ONE vector reduction per
+//          record, into the block's step histogram S[i4][m] (prefix-summed later in fp64);
+//   A4-A6  the paper's "thread = energy, thread-local accumulation" restricted to the
+//          window: lanes OWN energy bins and keep 2*MB sums (DOS and in-window N) in registers.  A warp
+//          is NG groups of GL lanes; a group owns GL consecutive bins (a "chunk") at a time.  Which
+//          records overlap which chunk is a bitmap built with warp ballots; the (record, chunk) entries
+//          of the whole item are split EVENLY over the NG groups (prefix sum over chunks), so the groups
+//          of a warp run the same number of steps.  Per step a group fetches its next record (a
+//          shared-memory broadcast), every lane evaluates Eq. 12/13/14 at its own omega and does the
+//          4 x MB projection as FMAs into its registers.  When a group leaves a chunk it adds its
+//          registers to the block's partial histogram (fp32 reductions in L2, one coalesced sector
+//          per orbital).
 // `tdos_merge` sums the block partials in fp64; `tdos_finalize` prefix-sums the step histogram in
 // fp64, scales by V and writes fp32 DOS and N (A7).
 #pragma once
@@ -40,7 +43,7 @@ struct MainParams {
     int nmb;                     // orbital blocks of MB
     int n_items;                 // ntx*nty*ntz*nb*nmb
     int unitW;                   // W == 1
-    float* partial;              // [gridDim.x][3][norb][nE]
+    float* partial;              // [gridDim.x] x { D[norb][nE], T[norb][nE], S[nE][norb] }
     unsigned long long* counters;   // [0] n_tb, [1] n_eval = #(tb, omega) with E1 < omega < E4
 };
 
@@ -74,39 +77,74 @@ __device__ __forceinline__ int locate_bin(const float* __restrict__ omega, int n
         }                                     \
     } while (0)
 
+// fire-and-forget fp32 reductions into global memory (performed in L2)
+__device__ __forceinline__ void red_add(float* addr, float v) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void red_add4(float* addr, float a, float b, float c, float d) {   // 16-byte aligned
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+// Per-warp shared-memory slice.
 template <int MB, int TX, int TY, int TZ>
-struct TileCfg {
+struct WarpCfg {
     static constexpr int PX = TX + 1, PY = TY + 1, PZ = TZ + 1;
     static constexpr int PK = PX * PY * PZ;          // k-points staged per tile
     static constexpr int NC = TX * TY * TZ;          // cubes per tile
     static constexpr int NTB = 6 * NC;               // (tetrahedron, band) records per item
-    static_assert(NTB % 8 == 0, "records are scanned 8 at a time");
-    static_assert(PK < 65536, "corner slots are 16-bit");
-    // dynamic shared memory layout (byte offsets, 16-byte aligned pieces first)
-    static constexpr size_t off_es = 0;                                   // float4 [NTB]
-    static constexpr size_t off_w = off_es + sizeof(float4) * NTB;        // float  [PK*MB]
-    static constexpr size_t off_cs = off_w + ((sizeof(float) * PK * MB + 15) / 16) * 16;   // uint2 [NTB]
-    static constexpr size_t off_rng = off_cs + sizeof(uint2) * NTB;       // uint32 [NTB]
-    static constexpr size_t off_e = off_rng + sizeof(uint32_t) * NTB;     // float  [PK]
-    static constexpr size_t off_s = off_e + ((sizeof(float) * PK + 15) / 16) * 16;   // float [MB*NT], then int[2]
-    static size_t bytes(int NT) { return off_s + sizeof(float) * MB * NT + 16; }
+    static constexpr int NWORD = (NTB + 31) / 32;    // 32-record words of a chunk's bitmap
+    static constexpr int BST = NWORD | 1;            // odd word stride between chunks: conflict-free column stores
+    static constexpr int NCH = 32;                   // chunks per pass (lane c keeps chunk c's counters)
+    static_assert(PK * MB < 65536, "corner slots are 16-bit");
+    static constexpr size_t a16(size_t x) { return (x + 15) / 16 * 16; }
+    static constexpr size_t off_es = 0;                                        // float4 [NWORD*32]
+    static constexpr size_t off_w = off_es + sizeof(float4) * NWORD * 32;      // float  [PK*MB]
+    static constexpr size_t off_cs = off_w + a16(sizeof(float) * PK * MB);     // uint2  [NWORD*32]
+    static constexpr size_t off_rng = off_cs + sizeof(uint2) * NWORD * 32;     // uint32 [NWORD*32]
+    static constexpr size_t off_e = off_rng + sizeof(uint32_t) * NWORD * 32;   // float  [PK]
+    static constexpr size_t off_bm = off_e + a16(sizeof(float) * PK);          // uint32 [NCH*BST]
+    static constexpr size_t off_off = off_bm + a16(sizeof(uint32_t) * NCH * BST);   // int [NCH+1]
+    static constexpr size_t bytes = off_off + a16(sizeof(int) * (NCH + 1));
 };
 
-template <int MB, int TX, int TY, int TZ, int NT>
-__global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
-    using Cfg = TileCfg<MB, TX, TY, TZ>;
-    constexpr int PX = Cfg::PX, PY = Cfg::PY, PK = Cfg::PK, NC = Cfg::NC, NTB = Cfg::NTB;
-    extern __shared__ __align__(16) unsigned char smem[];
-    float4* sEs = reinterpret_cast<float4*>(smem + Cfg::off_es);
-    float* sW = reinterpret_cast<float*>(smem + Cfg::off_w);
-    uint2* sCs = reinterpret_cast<uint2*>(smem + Cfg::off_cs);
-    uint32_t* sRng = reinterpret_cast<uint32_t*>(smem + Cfg::off_rng);
-    float* sE = reinterpret_cast<float*>(smem + Cfg::off_e);
-    float* sS = reinterpret_cast<float*>(smem + Cfg::off_s);
-    int* sMinMax = reinterpret_cast<int*>(sS + MB * NT);
+template <int MB>
+__device__ __forceinline__ void load_b(const float* __restrict__ bp, float (&b)[MB]) {
+    if constexpr (MB % 4 == 0) {
+#pragma unroll
+        for (int m4 = 0; m4 < MB; m4 += 4) {
+            const float4 v = *reinterpret_cast<const float4*>(bp + m4);
+            b[m4] = v.x; b[m4 + 1] = v.y; b[m4 + 2] = v.z; b[m4 + 3] = v.w;
+        }
+    } else if constexpr (MB == 2) {
+        const float2 v = *reinterpret_cast<const float2*>(bp);
+        b[0] = v.x; b[1] = v.y;
+    } else {
+#pragma unroll
+        for (int m = 0; m < MB; m++) b[m] = bp[m];
+    }
+}
 
-    const int tid = threadIdx.x;
-    const int lane = tid & 31;
+template <int MB, int TX, int TY, int TZ, int GL, int NWARP>
+__global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
+    using Cfg = WarpCfg<MB, TX, TY, TZ>;
+    constexpr int PX = Cfg::PX, PY = Cfg::PY, PK = Cfg::PK, NC = Cfg::NC, NTB = Cfg::NTB;
+    constexpr int NWORD = Cfg::NWORD, BST = Cfg::BST, NCH = Cfg::NCH;
+    constexpr int NG = 32 / GL;             // groups per warp
+    constexpr int PASS = NCH * GL;          // bins per pass
+    constexpr unsigned FULL = 0xffffffffu;
+    static_assert(GL == 4 || GL == 8 || GL == 16 || GL == 32, "group width");
+
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned char* base = smem + (size_t)warp * Cfg::bytes;
+    float4* sEs = reinterpret_cast<float4*>(base + Cfg::off_es);
+    float* sW = reinterpret_cast<float*>(base + Cfg::off_w);
+    uint2* sCs = reinterpret_cast<uint2*>(base + Cfg::off_cs);
+    uint32_t* sRng = reinterpret_cast<uint32_t*>(base + Cfg::off_rng);
+    float* sE = reinterpret_cast<float*>(base + Cfg::off_e);
+    uint32_t* sBm = reinterpret_cast<uint32_t*>(base + Cfg::off_bm);
+    int* sOff = reinterpret_cast<int*>(base + Cfg::off_off);
+
     const int nE = p.nE;
     const float* __restrict__ omega = p.omega;
     const float om0 = __ldg(omega);
@@ -115,11 +153,21 @@ __global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
         const float span = __ldg(omega + nE - 1) - om0;
         if (span > 0.0f) inv_dom = (float)(nE - 1) / span;
     }
-    float* part = p.partial + (size_t)blockIdx.x * 3 * p.norb * nE;   // written and re-read: no __restrict__
     const size_t qstride = (size_t)p.norb * nE;
+    float* partD = p.partial + (size_t)blockIdx.x * 3 * qstride;
+    float* partT = partD + qstride;
+    float* partS = partT + qstride;                               // [nE][norb]
+    const bool s_vec4 = (MB % 4 == 0) && (p.norb % 4 == 0);      // 16-byte aligned vector reductions into S
+    const bool w_vec4 = (MB % 4 == 0) && !p.unitW && p.sWm == 1 && (p.norb % 4 == 0) &&
+                        ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
 
-    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
-        // ---- decode the work item
+    const int g = lane / GL, gl = lane % GL;
+    unsigned long long cnt_tb = 0, cnt_ev = 0;
+    const float qnan = __int_as_float(0x7fc00000);
+
+    const int gwarp = blockIdx.x * NWARP + warp, nwarps = gridDim.x * NWARP;
+    for (int item = gwarp; item < p.n_items; item += nwarps) {
+        // ---- decode the work item (orbital block, band fastest: neighbouring warps share the tile's lines)
         int r = item;
         const int mb = r % p.nmb; r /= p.nmb;
         const int n = r % p.nb; r /= p.nb;
@@ -129,27 +177,37 @@ __global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
         const int x0 = tx * TX, y0 = ty * TY, z0 = p.z_lo + tz * TZ;
         const int m0 = mb * MB;
 
-        if (tid == 0) { sMinMax[0] = 0x7fffffff; sMinMax[1] = -1; }
-
         // ---- A1/A2: stage the tile (periodic wrap), E then W
-        for (int q = tid; q < PK; q += NT) {
+        for (int q = lane; q < PK; q += 32) {
             const int px = q % PX, py = (q / PX) % PY, pz = q / (PX * PY);
             const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
             const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
             sE[q] = __ldg(p.E + ik * p.sEk + (long long)n * p.sEn);
         }
         if (p.unitW) {
-            for (int q = tid; q < PK * MB; q += NT) sW[q] = ((q % MB) + m0 < p.norb) ? 1.0f : 0.0f;
-        } else if (p.sWm == 1) {   // orbitals contiguous (AoS): m fastest across threads
-            for (int q = tid; q < PK * MB; q += NT) {
+            for (int q = lane; q < PK * MB; q += 32) sW[q] = ((q % MB) + m0 < p.norb) ? 1.0f : 0.0f;
+        } else if (w_vec4) {       // orbitals contiguous (AoS), whole float4s
+            constexpr int Q4 = (MB >= 4) ? MB / 4 : 1;
+            for (int q = lane; q < PK * Q4; q += 32) {
+                const int part = q % Q4, k = q / Q4;
+                const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
+                const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
+                const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
+                float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (m0 + 4 * part < p.norb)
+                    v = __ldg(reinterpret_cast<const float4*>(p.W + ik * p.sWk + (long long)n * p.sWn + m0 + 4 * part));
+                *reinterpret_cast<float4*>(sW + k * MB + 4 * part) = v;
+            }
+        } else if (p.sWm == 1) {   // orbitals contiguous (AoS): m fastest across lanes
+            for (int q = lane; q < PK * MB; q += 32) {
                 const int m = q % MB, k = q / MB;
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
                 sW[k * MB + m] = (m0 + m < p.norb) ? __ldg(p.W + ik * p.sWk + (long long)n * p.sWn + (m0 + m)) : 0.0f;
             }
-        } else {                   // k contiguous (SoA): k fastest across threads
-            for (int q = tid; q < PK * MB; q += NT) {
+        } else {                   // k contiguous (SoA): k fastest across lanes
+            for (int q = lane; q < PK * MB; q += 32) {
                 const int k = q % PK, m = q / PK;
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
@@ -159,18 +217,21 @@ __global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
                                      : 0.0f;
             }
         }
-        __syncthreads();
+        __syncwarp();
 
-        // ---- A2/A3: one thread per (tetrahedron, band): sort, window, record
-        {
-            int lmin = 0x7fffffff, lmax = -1;
-            unsigned cnt_tb = 0, cnt_ev = 0;
-            for (int t = tid; t < NTB; t += NT) {
+        // ---- A2/A3 (+ Eq. 15): lane = (tetrahedron, band) record: sort, window, step histogram
+        int lmin = 0x7fffffff, lmax = -1;
+#pragma unroll 1
+        for (int wd = 0; wd < NWORD; ++wd) {
+            const int t = wd * 32 + lane;
+            uint32_t rng = 0;   // i1 = i4 = 0: empty window
+            float e0 = 0.f, e1 = 0.f, e2 = 0.f, e3 = 0.f;
+            unsigned c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+            if (t < NTB) {
                 const int tet = t / NC, cube = t - tet * NC;
                 const int cx = cube % TX, cy = (cube / TX) % TY, cz = cube / (TX * TY);
                 const bool valid = (x0 + cx < p.N1) && (y0 + cy < p.N2) && (z0 + cz < p.z_hi);
                 const int cbase = cx + PX * (cy + PY * cz);
-                unsigned c0, c1, c2, c3;
                 {
                     const int a0 = kTableI[tet][0], a1 = kTableI[tet][1], a2 = kTableI[tet][2], a3 = kTableI[tet][3];
                     c0 = cbase + (a0 & 1) + PX * (((a0 >> 1) & 1) + PY * (a0 >> 2));
@@ -178,159 +239,217 @@ __global__ void __launch_bounds__(NT) tdos_main(const MainParams p) {
                     c2 = cbase + (a2 & 1) + PX * (((a2 >> 1) & 1) + PY * (a2 >> 2));
                     c3 = cbase + (a3 & 1) + PX * (((a3 >> 1) & 1) + PY * (a3 >> 2));
                 }
-                float e0 = sE[c0], e1 = sE[c1], e2 = sE[c2], e3 = sE[c3];
+                e0 = sE[c0]; e1 = sE[c1]; e2 = sE[c2]; e3 = sE[c3];
                 TDOS_CSWAP(e0, e1, c0, c1);
                 TDOS_CSWAP(e2, e3, c2, c3);
                 TDOS_CSWAP(e0, e2, c0, c2);
                 TDOS_CSWAP(e1, e3, c1, c3);
                 TDOS_CSWAP(e1, e2, c1, c2);
-                uint32_t rng = 0xffffffffu;
+                c0 *= MB; c1 *= MB; c2 *= MB; c3 *= MB;   // float offsets into sW
                 if (valid) {
                     const int i1 = locate_bin<true>(omega, nE, om0, inv_dom, e0);      // first omega > E1
                     const int i4 = (e3 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e3) : i1;   // first omega >= E4 (and > E1)
                     rng = (uint32_t)i1 | ((uint32_t)i4 << 16);
-                    cnt_tb += 1;
-                    cnt_ev += (unsigned)(i4 - i1);
-                    if (i1 < nE) {
+                    if (mb == 0) {   // work counters (exact integers; bench.py's flop count uses them)
+                        cnt_tb += 1;
+                        cnt_ev += (unsigned)(i4 - i1);
+                    }
+                    if (i1 < i4) {
                         lmin = min(lmin, i1);
-                        lmax = max(lmax, min(i4, nE - 1));
+                        lmax = max(lmax, i4 - 1);
                     }
-                }
-                sEs[t] = make_float4(e0, e1, e2, e3);
-                sCs[t] = make_uint2(c0 | (c1 << 16), c2 | (c3 << 16));
-                sRng[t] = rng;
-            }
-            lmin = __reduce_min_sync(0xffffffffu, lmin);
-            lmax = __reduce_max_sync(0xffffffffu, lmax);
-            if (lane == 0 && lmax >= 0) {
-                atomicMin(&sMinMax[0], lmin);
-                atomicMax(&sMinMax[1], lmax);
-            }
-            if (mb == 0) {   // work counters (exact integers; bench.py's flop count uses them)
-                cnt_tb = __reduce_add_sync(0xffffffffu, cnt_tb);
-                cnt_ev = __reduce_add_sync(0xffffffffu, cnt_ev);
-                if (lane == 0) {
-                    atomicAdd(p.counters + 0, (unsigned long long)cnt_tb);
-                    atomicAdd(p.counters + 1, (unsigned long long)cnt_ev);
-                }
-            }
-        }
-        __syncthreads();
-        const int bmin = sMinMax[0], bmax = sMinMax[1];
-
-        // ---- passes of NT bins over the tile's energy span
-        for (int pb = bmin; pb <= bmax; pb += NT) {
-            for (int q = tid; q < MB * NT; q += NT) sS[q] = 0.0f;
-            __syncthreads();
-
-            // Eq. 15 (A6): tetrahedra lying entirely below omega contribute V*sum_l b_l to every
-            // higher bin: one add into the step histogram at bin i4
-            for (int t = tid; t < NTB; t += NT) {
-                const int i4 = (int)(sRng[t] >> 16);
-                if (i4 < nE && i4 >= pb && i4 < pb + NT) {
-                    const uint2 cs = sCs[t];
-                    const float* b0 = sW + (cs.x & 0xffffu) * MB;
-                    const float* b1 = sW + (cs.x >> 16) * MB;
-                    const float* b2 = sW + (cs.y & 0xffffu) * MB;
-                    const float* b3 = sW + (cs.y >> 16) * MB;
+                    // Eq. 15 (A6): a tetrahedron lying entirely below omega contributes V*sum_l b_l to
+                    // every bin >= i4: one add into the step histogram at bin i4
+                    if (i4 < nE) {
+                        float b0[MB], b1[MB], b2[MB], b3[MB];
+                        load_b<MB>(sW + c0, b0);
+                        load_b<MB>(sW + c1, b1);
+                        load_b<MB>(sW + c2, b2);
+                        load_b<MB>(sW + c3, b3);
+                        float* dst = partS + (size_t)i4 * p.norb + m0;
+                        if (s_vec4) {
+                            if constexpr (MB % 4 == 0) {
 #pragma unroll
-                    for (int m = 0; m < MB; m++) atomicAdd(&sS[m * NT + (i4 - pb)], (b0[m] + b1[m]) + (b2[m] + b3[m]));
-                }
-            }
-
-            // A4-A6: thread = energy bin, group of 8 lanes = 8 consecutive bins
-            const int bin = pb + tid;
-            const float om = (bin < nE) ? __ldg(omega + bin) : -INFINITY;
-            float accD[MB], accT[MB];
-#pragma unroll
-            for (int m = 0; m < MB; m++) accD[m] = accT[m] = 0.0f;
-
-            const int gsh = lane & 24;
-            const unsigned gmask = 0xffu << gsh;
-            const int gl = lane & 7;
-            const int gb = pb + (tid & ~7);
-            if (gb <= bmax) {
-                int t0 = 0, base = 0;
-                unsigned mask = 0;
-                for (;;) {
-                    while (mask == 0 && t0 < NTB) {
-                        const uint32_t rr = sRng[t0 + gl];
-                        const int i1 = (int)(rr & 0xffffu), i4 = (int)(rr >> 16);
-                        const bool hit = (i1 <= gb + 7) && (i4 > gb) && (i1 < i4);
-                        mask = (__ballot_sync(gmask, hit) >> gsh) & 0xffu;
-                        base = t0;
-                        t0 += 8;
-                    }
-                    if (mask == 0) break;
-                    const int t = base + __ffs(mask) - 1;
-                    mask &= mask - 1;
-
-                    const float4 es = sEs[t];
-                    const uint2 cs = sCs[t];
-                    float w[4], dw[4];
-                    if (om > es.x && om < es.w) {
-                        corner_weights_in_window(es.x, es.y, es.z, es.w, om, w, dw);
-                    } else {
-#pragma unroll
-                        for (int l = 0; l < 4; l++) w[l] = dw[l] = 0.0f;
-                    }
-                    const unsigned cc[4] = {cs.x & 0xffffu, cs.x >> 16, cs.y & 0xffffu, cs.y >> 16};
-#pragma unroll
-                    for (int l = 0; l < 4; l++) {
-                        const float* bp = sW + cc[l] * MB;
-                        if constexpr (MB % 4 == 0) {
-#pragma unroll
-                            for (int m4 = 0; m4 < MB; m4 += 4) {
-                                const float4 b = *reinterpret_cast<const float4*>(bp + m4);
-                                accD[m4 + 0] = fmaf(b.x, dw[l], accD[m4 + 0]);
-                                accD[m4 + 1] = fmaf(b.y, dw[l], accD[m4 + 1]);
-                                accD[m4 + 2] = fmaf(b.z, dw[l], accD[m4 + 2]);
-                                accD[m4 + 3] = fmaf(b.w, dw[l], accD[m4 + 3]);
-                                accT[m4 + 0] = fmaf(b.x, w[l], accT[m4 + 0]);
-                                accT[m4 + 1] = fmaf(b.y, w[l], accT[m4 + 1]);
-                                accT[m4 + 2] = fmaf(b.z, w[l], accT[m4 + 2]);
-                                accT[m4 + 3] = fmaf(b.w, w[l], accT[m4 + 3]);
+                                for (int m4 = 0; m4 < MB; m4 += 4)
+                                    if (m0 + m4 < p.norb)
+                                        red_add4(dst + m4, (b0[m4] + b1[m4]) + (b2[m4] + b3[m4]),
+                                                 (b0[m4 + 1] + b1[m4 + 1]) + (b2[m4 + 1] + b3[m4 + 1]),
+                                                 (b0[m4 + 2] + b1[m4 + 2]) + (b2[m4 + 2] + b3[m4 + 2]),
+                                                 (b0[m4 + 3] + b1[m4 + 3]) + (b2[m4 + 3] + b3[m4 + 3]));
                             }
                         } else {
 #pragma unroll
-                            for (int m = 0; m < MB; m++) {
-                                const float b = bp[m];
-                                accD[m] = fmaf(b, dw[l], accD[m]);
-                                accT[m] = fmaf(b, w[l], accT[m]);
-                            }
+                            for (int m = 0; m < MB; m++)
+                                if (m0 + m < p.norb) red_add(dst + m, (b0[m] + b1[m]) + (b2[m] + b3[m]));
                         }
                     }
                 }
             }
-            __syncthreads();   // step histogram complete
+            sEs[t] = make_float4(e0, e1, e2, e3);
+            sCs[t] = make_uint2(c0 | (c1 << 16), c2 | (c3 << 16));
+            sRng[t] = rng;
+        }
+        lmin = __reduce_min_sync(FULL, lmin);
+        lmax = __reduce_max_sync(FULL, lmax);
+        __syncwarp();
 
-            // ---- flush this pass into the block's private partial histogram
-            if (bin <= bmax) {   // bmax <= nE-1
+        // ---- passes of PASS bins over the tile's energy span
+#pragma unroll 1
+        for (int pb = lmin; pb <= lmax; pb += PASS) {
+            const int pe = pb + PASS;
+            // -- which records overlap which chunk: bm[c][wd] bit j <=> record 32*wd+j has bins in chunk c
+            int mycnt = 0;   // lane c: entries of chunk c
+#pragma unroll 1
+            for (int wd = 0; wd < NWORD; ++wd) {
+                const uint32_t rr = sRng[wd * 32 + lane];
+                const int i1 = (int)(rr & 0xffffu), i4 = (int)(rr >> 16);
+                const bool has = (i1 < i4) && (i4 > pb) && (i1 < pe);
+                int c1 = NCH, c2 = -1;
+                if (has) {
+                    c1 = (max(i1, pb) - pb) / GL;
+                    c2 = (min(i4, pe) - 1 - pb) / GL;
+                }
+                const int cmin = __reduce_min_sync(FULL, c1);
+                const int cmax = __reduce_max_sync(FULL, c2);
+                uint32_t myword = 0;
+                for (int c = cmin; c <= cmax; ++c) {
+                    const uint32_t b = __ballot_sync(FULL, c1 <= c && c <= c2);
+                    if (lane == c) myword = b;
+                }
+                sBm[lane * BST + wd] = myword;
+                mycnt += __popc(myword);
+            }
+            // -- exclusive prefix over chunks: the item's entries as one flat list
+            int incl = mycnt;
 #pragma unroll
-                for (int m = 0; m < MB; m++) {
-                    if (m0 + m < p.norb) {
-                        float* d = part + (size_t)(m0 + m) * nE + bin;
-                        d[0] += accD[m];
-                        d[qstride] += accT[m];
-                        d[2 * qstride] += sS[m * NT + tid];
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(FULL, incl, d);
+                if (lane >= d) incl += v;
+            }
+            const int off = incl - mycnt;
+            const int T = __shfl_sync(FULL, incl, 31);
+            sOff[lane] = off;
+            __syncwarp();
+            if (T == 0) continue;
+
+            // -- even split of the flat list over the NG groups: group g takes entries [g*q, g*q + rem)
+            const int q = (T + NG - 1) / NG;
+            const int start = g * q;
+            int rem = min(max(T - start, 0), q);
+            const bool worked = rem > 0;
+            int c = 0;
+#pragma unroll
+            for (int gg = 0; gg < NG; ++gg) {
+                const uint32_t b = __ballot_sync(FULL, off <= gg * q);   // monotone: bits 0..c*
+                if (gg == g) c = 31 - __clz(b);
+            }
+            int w = 0;
+            uint32_t m = 0;
+            if (worked) {
+                int skip = start - sOff[c];
+                m = sBm[c * BST];
+                int pc = __popc(m);
+                while (skip >= pc) {
+                    skip -= pc;
+                    ++w;
+                    m = sBm[c * BST + w];
+                    pc = __popc(m);
+                }
+                for (; skip > 0; --skip) m &= m - 1;
+            }
+            int bin = pb + c * GL + gl;
+            float om = (bin < nE) ? __ldg(omega + bin) : qnan;
+
+            float accD[MB], accT[MB];
+#pragma unroll
+            for (int mm = 0; mm < MB; mm++) accD[mm] = accT[mm] = 0.0f;
+
+            auto flush = [&]() {   // this group's registers -> the block's partial histogram
+                if (bin < nE) {
+#pragma unroll
+                    for (int mm = 0; mm < MB; mm++) {
+                        if (m0 + mm < p.norb) {
+                            red_add(partD + (size_t)(m0 + mm) * nE + bin, accD[mm]);
+                            red_add(partT + (size_t)(m0 + mm) * nE + bin, accT[mm]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int mm = 0; mm < MB; mm++) accD[mm] = accT[mm] = 0.0f;
+            };
+
+            // -- A4-A6: every group walks its share of the list; lanes own bins
+#pragma unroll 1
+            for (int step = 0; step < q; ++step) {
+                if (rem > 0) {
+                    while (m == 0) {   // next word / next chunk (uniform within the group)
+                        ++w;
+                        if (w == NWORD) {
+                            flush();
+                            ++c;
+                            w = 0;
+                            bin += GL;
+                            om = (bin < nE) ? __ldg(omega + bin) : qnan;
+                        }
+                        m = sBm[c * BST + w];
+                    }
+                    const int t = w * 32 + __ffs(m) - 1;
+                    m &= m - 1;
+                    --rem;
+
+                    const float4 es = sEs[t];
+                    const uint2 cs = sCs[t];
+                    float wv[4], dw[4];
+                    if (om > es.x && om < es.w) {
+                        corner_weights_in_window(es.x, es.y, es.z, es.w, om, wv, dw);
+                    } else {
+#pragma unroll
+                        for (int l = 0; l < 4; l++) wv[l] = dw[l] = 0.0f;
+                    }
+                    const unsigned cc[4] = {cs.x & 0xffffu, cs.x >> 16, cs.y & 0xffffu, cs.y >> 16};
+#pragma unroll
+                    for (int l = 0; l < 4; l++) {
+                        float b[MB];
+                        load_b<MB>(sW + cc[l], b);
+#pragma unroll
+                        for (int mm = 0; mm < MB; mm++) {
+                            accD[mm] = fmaf(b[mm], dw[l], accD[mm]);
+                            accT[mm] = fmaf(b[mm], wv[l], accT[mm]);
+                        }
                     }
                 }
             }
-            __syncthreads();
+            if (worked) flush();
+            __syncwarp();   // the next pass rewrites the bitmaps
         }
-        __syncthreads();   // smem is reused by the next item
+        __syncwarp();   // the next item rewrites the slice
+    }
+
+    cnt_tb = __reduce_add_sync(FULL, (unsigned)cnt_tb);   // per warp < 2^32
+    unsigned long long ev = cnt_ev;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) ev += __shfl_xor_sync(FULL, ev, d);
+    if (lane == 0 && (cnt_tb | ev)) {
+        atomicAdd(p.counters + 0, cnt_tb);
+        atomicAdd(p.counters + 1, ev);
     }
 }
 
-// A7a: sum the block partials in fp64.  out[j] = sum_c partial[c][j], j < n (= 3*norb*nE)
-__global__ void __launch_bounds__(256) tdos_merge(const float* __restrict__ partial, int nblk, size_t n, double* __restrict__ out) {
+// A7a: sum the block partials in fp64.  out[3][norb][nE]; the step histogram is stored [nE][norb] per block.
+__global__ void __launch_bounds__(256) tdos_merge(const float* __restrict__ partial, int nblk, int norb, int nE,
+                                                  double* __restrict__ out) {
+    const size_t q = (size_t)norb * nE, n = 3 * q;
     for (size_t j = blockIdx.x * (size_t)blockDim.x + threadIdx.x; j < n; j += (size_t)gridDim.x * blockDim.x) {
+        size_t src = j;
+        if (j >= 2 * q) {
+            const size_t r = j - 2 * q, m = r / nE, i = r - m * nE;
+            src = 2 * q + i * norb + m;
+        }
         double s = 0.0;
-        for (int c = 0; c < nblk; c++) s += (double)partial[(size_t)c * n + j];
+        for (int c = 0; c < nblk; c++) s += (double)partial[(size_t)c * n + src];
         out[j] = s;
     }
 }
-
 // A7b: one block per orbital.  dos = V*D ; nos = V*(T + inclusive prefix over omega of S), fp64 inside.
 __global__ void __launch_bounds__(1024) tdos_finalize(const double* __restrict__ part, int norb, int nE, double V,
                                                       float* __restrict__ dos, float* __restrict__ nos) {

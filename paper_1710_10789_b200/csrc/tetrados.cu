@@ -34,23 +34,25 @@ typedef void (*main_kernel_t)(const MainParams);
 
 struct Variant {
     main_kernel_t fn;
-    int MB, TX, TY, TZ, NT;
+    int MB, TX, TY, TZ, GL, NWARP;
     size_t smem;
 };
 
-template <int MB, int TX, int TY, int TZ, int NT>
+template <int MB, int TX, int TY, int TZ, int GL, int NWARP>
 Variant make_variant() {
-    return Variant{tdos::tdos_main<MB, TX, TY, TZ, NT>, MB, TX, TY, TZ, NT, tdos::TileCfg<MB, TX, TY, TZ>::bytes(NT)};
+    return Variant{tdos::tdos_main<MB, TX, TY, TZ, GL, NWARP>, MB, TX, TY, TZ, GL, NWARP,
+                   (size_t)NWARP * tdos::WarpCfg<MB, TX, TY, TZ>::bytes};
 }
 
 // orbital-block width: the smallest of 1, 2, 4, 8 that holds norb (8 for norb > 8, several blocks)
 int pick_mb(int norb) { return norb <= 1 ? 1 : norb <= 2 ? 2 : norb <= 4 ? 4 : 8; }
 
-// Tile shapes compiled in.  TDOS_TILE=<index> selects another one for experiments.
+// Configurations compiled in: tile of cubes per warp, lanes per group, warps per block.
+// TDOS_TILE=<index> selects another one for experiments.
 template <int MB>
 std::vector<Variant> variants_for() {
-    return {make_variant<MB, 8, 8, 4, 256>(), make_variant<MB, 8, 8, 8, 256>(), make_variant<MB, 4, 4, 8, 128>(),
-            make_variant<MB, 8, 4, 4, 128>(), make_variant<MB, 16, 8, 2, 256>()};
+    return {make_variant<MB, 4, 4, 4, 8, 12>(), make_variant<MB, 4, 4, 4, 4, 12>(), make_variant<MB, 4, 4, 2, 8, 24>(),
+            make_variant<MB, 4, 4, 2, 4, 24>(), make_variant<MB, 8, 4, 2, 8, 12>()};
 }
 
 std::vector<Variant> variants(int MB) {
@@ -162,7 +164,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
 
     cudaError_t e = cudaFuncSetAttribute(p->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->var.smem);
     if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->blocks_per_sm, p->var.fn, p->var.NT, p->var.smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->blocks_per_sm, p->var.fn, p->var.NWARP * 32, p->var.smem);
     if (e != cudaSuccess || p->blocks_per_sm < 1) {
         int rc = (e != cudaSuccess) ? cuda_fail(e, "kernel setup") : TDOS_ECUDA;
         delete p;
@@ -244,15 +246,16 @@ static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int lay
     mp.counters = p->counters;
 
     const size_t hist = (size_t)3 * p->norb * nE;
-    const int grid = (int)((items < p->grid) ? (items > 0 ? items : 1) : p->grid);
+    const long long blocks_needed = (items + v.NWARP - 1) / v.NWARP;
+    const int grid = (int)((blocks_needed < p->grid) ? (blocks_needed > 0 ? blocks_needed : 1) : p->grid);
     CK(cudaMemsetAsync(p->partial, 0, hist * grid * sizeof(float), st));
     CK(cudaMemsetAsync(p->counters, 0, 2 * sizeof(unsigned long long), st));
     CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
-    v.fn<<<grid, v.NT, v.smem, st>>>(mp);
+    v.fn<<<grid, v.NWARP * 32, v.smem, st>>>(mp);
     CK(cudaGetLastError());
     CK(cudaEventRecord(p->ring[p->cur_slot][1], st));
     const int mblocks = (int)((hist + 255) / 256);
-    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, grid, hist, part_out);
+    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, grid, p->norb, nE, part_out);
     CK(cudaGetLastError());
     p->last_items = items;
     p->last_launches = 2;
@@ -368,7 +371,7 @@ int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, f
 int tdos_plan_info(const tdos_plan* p, long long what[8]) {
     if (!p || !what) return TDOS_EINVAL;
     what[0] = p->grid;
-    what[1] = p->var.NT;
+    what[1] = p->var.NWARP * 32;
     what[2] = (long long)p->var.smem;
     what[3] = p->last_items;
     what[4] = p->last_launches;
