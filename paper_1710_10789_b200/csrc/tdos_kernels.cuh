@@ -85,6 +85,10 @@ __device__ __forceinline__ void red_add4(float* addr, float a, float b, float c,
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
+__device__ __forceinline__ void red_add2(float* addr, float a, float b) {   // 8-byte aligned
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(a), "f"(b) : "memory");
+}
+
 // Per-warp shared-memory slice.
 template <int MB, int TX, int TY, int TZ>
 struct WarpCfg {
@@ -95,16 +99,18 @@ struct WarpCfg {
     static constexpr int NWORD = (NTB + 31) / 32;    // 32-record words of a chunk's bitmap
     static constexpr int BST = NWORD | 1;            // odd word stride between chunks: conflict-free column stores
     static constexpr int NCH = 32;                   // chunks per pass (lane c keeps chunk c's counters)
-    static_assert(PK * MB < 65536, "corner slots are 16-bit");
+    static constexpr int WST = (MB >= 4) ? MB + 4 : MB;   // floats between k-points in sW: 48-byte rows spread the banks
+    static_assert(NWORD <= 32, "word mask is 32 bits");
+    static_assert(PK * WST < 65536, "corner slots are 16-bit");
     static constexpr size_t a16(size_t x) { return (x + 15) / 16 * 16; }
     static constexpr size_t off_es = 0;                                        // float4 [NWORD*32]
-    static constexpr size_t off_w = off_es + sizeof(float4) * NWORD * 32;      // float  [PK*MB]
-    static constexpr size_t off_cs = off_w + a16(sizeof(float) * PK * MB);     // uint2  [NWORD*32]
+    static constexpr size_t off_w = off_es + sizeof(float4) * NWORD * 32;      // float  [PK*WST]
+    static constexpr size_t off_cs = off_w + a16(sizeof(float) * PK * WST);    // uint2  [NWORD*32]
     static constexpr size_t off_rng = off_cs + sizeof(uint2) * NWORD * 32;     // uint32 [NWORD*32]
     static constexpr size_t off_e = off_rng + sizeof(uint32_t) * NWORD * 32;   // float  [PK]
     static constexpr size_t off_bm = off_e + a16(sizeof(float) * PK);          // uint32 [NCH*BST]
-    static constexpr size_t off_off = off_bm + a16(sizeof(uint32_t) * NCH * BST);   // int [NCH+1]
-    static constexpr size_t bytes = off_off + a16(sizeof(int) * (NCH + 1));
+    static constexpr size_t off_off = off_bm + a16(sizeof(uint32_t) * NCH * BST);   // int [NCH], uint32 wordmask [NCH]
+    static constexpr size_t bytes = off_off + a16(sizeof(int) * 2 * NCH);
 };
 
 template <int MB>
@@ -124,15 +130,94 @@ __device__ __forceinline__ void load_b(const float* __restrict__ bp, float (&b)[
     }
 }
 
+// Register accumulators of one lane: two adjacent energy bins (a, b) x MB orbitals x {DOS, in-window N}.
+// MB >= 2: packed along the orbitals, acc[bin][m/2] = (m, m+1);  MB == 1: packed along the bins.
+template <int MB>
+struct Acc {
+    static constexpr int NP = (MB >= 2) ? MB / 2 : 1;
+    f2 D[2][NP], T[2][NP];
+    __device__ __forceinline__ void zero() {
+#pragma unroll
+        for (int h = 0; h < 2; h++)
+#pragma unroll
+            for (int j = 0; j < NP; j++) D[h][j] = T[h][j] = make_float2(0.f, 0.f);
+    }
+    // acc += b[l][:] * (dw[l], w[l]) for the 4 sorted corners; w, dw packed along the two bins
+    __device__ __forceinline__ void project(const float* __restrict__ sW, const unsigned (&cc)[4], const f2 (&w)[4],
+                                            const f2 (&dw)[4]) {
+#pragma unroll
+        for (int l = 0; l < 4; l++) {
+            float b[MB];
+            load_b<MB>(sW + cc[l], b);
+            if constexpr (MB >= 2) {
+                const f2 da = dup(dw[l].x), db = dup(dw[l].y), wa = dup(w[l].x), wb = dup(w[l].y);
+#pragma unroll
+                for (int j = 0; j < NP; j++) {
+                    const f2 bb = make_float2(b[2 * j], b[2 * j + 1]);
+                    D[0][j] = fma2(bb, da, D[0][j]);
+                    D[1][j] = fma2(bb, db, D[1][j]);
+                    T[0][j] = fma2(bb, wa, T[0][j]);
+                    T[1][j] = fma2(bb, wb, T[1][j]);
+                }
+            } else {
+                const f2 bb = dup(b[0]);
+                D[0][0] = fma2(bb, dw[l], D[0][0]);
+                T[0][0] = fma2(bb, w[l], T[0][0]);
+            }
+        }
+    }
+    // add to the block's partial histogram rows [bin][ D(norb) | T(norb) | S(norb) ] and clear
+    __device__ __forceinline__ void flush(float* __restrict__ part, int bin0, int nE, int norb, int m0, bool vec4) {
+        if constexpr (MB >= 2) {
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                if (bin0 + h < nE) {
+                    float* row = part + (size_t)(bin0 + h) * 3 * norb + m0;
+                    if (vec4) {
+                        if constexpr (MB % 4 == 0) {
+#pragma unroll
+                            for (int j = 0; j < NP; j += 2) {
+                                if (m0 + 2 * j < norb) {
+                                    red_add4(row + 2 * j, D[h][j].x, D[h][j].y, D[h][j + 1].x, D[h][j + 1].y);
+                                    red_add4(row + norb + 2 * j, T[h][j].x, T[h][j].y, T[h][j + 1].x, T[h][j + 1].y);
+                                }
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < NP; j++) {
+                            if (m0 + 2 * j < norb) { red_add(row + 2 * j, D[h][j].x); red_add(row + norb + 2 * j, T[h][j].x); }
+                            if (m0 + 2 * j + 1 < norb) { red_add(row + 2 * j + 1, D[h][j].y); red_add(row + norb + 2 * j + 1, T[h][j].y); }
+                        }
+                    }
+                }
+            }
+        } else {
+            if (bin0 < nE) {
+                float* row = part + (size_t)bin0 * 3 * norb + m0;
+                red_add(row, D[0][0].x);
+                red_add(row + norb, T[0][0].x);
+            }
+            if (bin0 + 1 < nE) {
+                float* row = part + (size_t)(bin0 + 1) * 3 * norb + m0;
+                red_add(row, D[0][0].y);
+                red_add(row + norb, T[0][0].y);
+            }
+        }
+        zero();
+    }
+};
+
 template <int MB, int TX, int TY, int TZ, int GL, int NWARP>
 __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     using Cfg = WarpCfg<MB, TX, TY, TZ>;
     constexpr int PX = Cfg::PX, PY = Cfg::PY, PK = Cfg::PK, NC = Cfg::NC, NTB = Cfg::NTB;
-    constexpr int NWORD = Cfg::NWORD, BST = Cfg::BST, NCH = Cfg::NCH;
+    constexpr int NWORD = Cfg::NWORD, BST = Cfg::BST, NCH = Cfg::NCH, WST = Cfg::WST;
     constexpr int NG = 32 / GL;             // groups per warp
-    constexpr int PASS = NCH * GL;          // bins per pass
+    constexpr int CH = 2 * GL;              // bins per chunk: every lane owns two adjacent bins
+    constexpr int PASS = NCH * CH;          // bins per pass
     constexpr unsigned FULL = 0xffffffffu;
-    static_assert(GL == 4 || GL == 8 || GL == 16 || GL == 32, "group width");
+    static_assert(GL == 2 || GL == 4 || GL == 8 || GL == 16, "group width");
 
     extern __shared__ __align__(16) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -144,8 +229,10 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     float* sE = reinterpret_cast<float*>(base + Cfg::off_e);
     uint32_t* sBm = reinterpret_cast<uint32_t*>(base + Cfg::off_bm);
     int* sOff = reinterpret_cast<int*>(base + Cfg::off_off);
+    uint32_t* sWm = reinterpret_cast<uint32_t*>(sOff + NCH);
 
     const int nE = p.nE;
+    const int norb = p.norb;
     const float* __restrict__ omega = p.omega;
     const float om0 = __ldg(omega);
     float inv_dom = 0.0f;
@@ -153,12 +240,9 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
         const float span = __ldg(omega + nE - 1) - om0;
         if (span > 0.0f) inv_dom = (float)(nE - 1) / span;
     }
-    const size_t qstride = (size_t)p.norb * nE;
-    float* partD = p.partial + (size_t)blockIdx.x * 3 * qstride;
-    float* partT = partD + qstride;
-    float* partS = partT + qstride;                               // [nE][norb]
-    const bool s_vec4 = (MB % 4 == 0) && (p.norb % 4 == 0);      // 16-byte aligned vector reductions into S
-    const bool w_vec4 = (MB % 4 == 0) && !p.unitW && p.sWm == 1 && (p.norb % 4 == 0) &&
+    float* part = p.partial + (size_t)blockIdx.x * 3 * norb * nE;   // rows [bin][ D | T | S ]
+    const bool vec4 = (MB % 4 == 0) && (norb % 4 == 0);          // 16-byte aligned vector reductions
+    const bool w_vec4 = (MB % 4 == 0) && !p.unitW && p.sWm == 1 && (norb % 4 == 0) &&
                         ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
 
     const int g = lane / GL, gl = lane % GL;
@@ -185,18 +269,18 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
             sE[q] = __ldg(p.E + ik * p.sEk + (long long)n * p.sEn);
         }
         if (p.unitW) {
-            for (int q = lane; q < PK * MB; q += 32) sW[q] = ((q % MB) + m0 < p.norb) ? 1.0f : 0.0f;
+            for (int q = lane; q < PK * MB; q += 32) sW[(q / MB) * WST + q % MB] = ((q % MB) + m0 < norb) ? 1.0f : 0.0f;
         } else if (w_vec4) {       // orbitals contiguous (AoS), whole float4s
             constexpr int Q4 = (MB >= 4) ? MB / 4 : 1;
             for (int q = lane; q < PK * Q4; q += 32) {
-                const int part = q % Q4, k = q / Q4;
+                const int part4 = q % Q4, k = q / Q4;
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
                 float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (m0 + 4 * part < p.norb)
-                    v = __ldg(reinterpret_cast<const float4*>(p.W + ik * p.sWk + (long long)n * p.sWn + m0 + 4 * part));
-                *reinterpret_cast<float4*>(sW + k * MB + 4 * part) = v;
+                if (m0 + 4 * part4 < norb)
+                    v = __ldg(reinterpret_cast<const float4*>(p.W + ik * p.sWk + (long long)n * p.sWn + m0 + 4 * part4));
+                *reinterpret_cast<float4*>(sW + k * WST + 4 * part4) = v;
             }
         } else if (p.sWm == 1) {   // orbitals contiguous (AoS): m fastest across lanes
             for (int q = lane; q < PK * MB; q += 32) {
@@ -204,7 +288,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
-                sW[k * MB + m] = (m0 + m < p.norb) ? __ldg(p.W + ik * p.sWk + (long long)n * p.sWn + (m0 + m)) : 0.0f;
+                sW[k * WST + m] = (m0 + m < norb) ? __ldg(p.W + ik * p.sWk + (long long)n * p.sWn + (m0 + m)) : 0.0f;
             }
         } else {                   // k contiguous (SoA): k fastest across lanes
             for (int q = lane; q < PK * MB; q += 32) {
@@ -212,14 +296,14 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
-                sW[k * MB + m] = (m0 + m < p.norb)
-                                     ? __ldg(p.W + ik * p.sWk + (long long)n * p.sWn + (long long)(m0 + m) * p.sWm)
-                                     : 0.0f;
+                sW[k * WST + m] = (m0 + m < norb)
+                                      ? __ldg(p.W + ik * p.sWk + (long long)n * p.sWn + (long long)(m0 + m) * p.sWm)
+                                      : 0.0f;
             }
         }
         __syncwarp();
 
-        // ---- A2/A3 (+ Eq. 15): lane = (tetrahedron, band) record: sort, window, step histogram
+        // ---- A2/A3 (+ Eq. 14/15 constants): lane = (tetrahedron, band) record: sort, window, step histogram
         int lmin = 0x7fffffff, lmax = -1;
 #pragma unroll 1
         for (int wd = 0; wd < NWORD; ++wd) {
@@ -245,10 +329,12 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 TDOS_CSWAP(e0, e2, c0, c2);
                 TDOS_CSWAP(e1, e3, c1, c3);
                 TDOS_CSWAP(e1, e2, c1, c2);
-                c0 *= MB; c1 *= MB; c2 *= MB; c3 *= MB;   // float offsets into sW
+                c0 *= WST; c1 *= WST; c2 *= WST; c3 *= WST;   // float offsets into sW
                 if (valid) {
                     const int i1 = locate_bin<true>(omega, nE, om0, inv_dom, e0);      // first omega > E1
-                    const int i4 = (e3 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e3) : i1;   // first omega >= E4 (and > E1)
+                    // first omega >= E3 / >= E4, and > E1 (test order G10)
+                    const int i3 = (e2 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e2) : i1;
+                    const int i4 = (e3 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e3) : i1;
                     rng = (uint32_t)i1 | ((uint32_t)i4 << 16);
                     if (mb == 0) {   // work counters (exact integers; bench.py's flop count uses them)
                         cnt_tb += 1;
@@ -258,20 +344,21 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                         lmin = min(lmin, i1);
                         lmax = max(lmax, i4 - 1);
                     }
-                    // Eq. 15 (A6): a tetrahedron lying entirely below omega contributes V*sum_l b_l to
-                    // every bin >= i4: one add into the step histogram at bin i4
-                    if (i4 < nE) {
+                    // Eq. 14c/e and Eq. 15 (A6): from the first omega >= E3 on, every corner carries the constant
+                    // V (Eq. 14 adds -C y/E_4j to it inside the window): one add of sum_l b_l into the
+                    // step histogram at bin i3
+                    if (i3 < nE) {
                         float b0[MB], b1[MB], b2[MB], b3[MB];
                         load_b<MB>(sW + c0, b0);
                         load_b<MB>(sW + c1, b1);
                         load_b<MB>(sW + c2, b2);
                         load_b<MB>(sW + c3, b3);
-                        float* dst = partS + (size_t)i4 * p.norb + m0;
-                        if (s_vec4) {
+                        float* dst = part + (size_t)i3 * 3 * norb + 2 * norb + m0;
+                        if (vec4) {
                             if constexpr (MB % 4 == 0) {
 #pragma unroll
                                 for (int m4 = 0; m4 < MB; m4 += 4)
-                                    if (m0 + m4 < p.norb)
+                                    if (m0 + m4 < norb)
                                         red_add4(dst + m4, (b0[m4] + b1[m4]) + (b2[m4] + b3[m4]),
                                                  (b0[m4 + 1] + b1[m4 + 1]) + (b2[m4 + 1] + b3[m4 + 1]),
                                                  (b0[m4 + 2] + b1[m4 + 2]) + (b2[m4 + 2] + b3[m4 + 2]),
@@ -280,7 +367,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                         } else {
 #pragma unroll
                             for (int m = 0; m < MB; m++)
-                                if (m0 + m < p.norb) red_add(dst + m, (b0[m] + b1[m]) + (b2[m] + b3[m]));
+                                if (m0 + m < norb) red_add(dst + m, (b0[m] + b1[m]) + (b2[m] + b3[m]));
                         }
                     }
                 }
@@ -298,7 +385,8 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
         for (int pb = lmin; pb <= lmax; pb += PASS) {
             const int pe = pb + PASS;
             // -- which records overlap which chunk: bm[c][wd] bit j <=> record 32*wd+j has bins in chunk c
-            int mycnt = 0;   // lane c: entries of chunk c
+            int mycnt = 0;          // lane c: entries of chunk c
+            uint32_t mywm = 0;      // lane c: non-empty words of chunk c
 #pragma unroll 1
             for (int wd = 0; wd < NWORD; ++wd) {
                 const uint32_t rr = sRng[wd * 32 + lane];
@@ -306,8 +394,8 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const bool has = (i1 < i4) && (i4 > pb) && (i1 < pe);
                 int c1 = NCH, c2 = -1;
                 if (has) {
-                    c1 = (max(i1, pb) - pb) / GL;
-                    c2 = (min(i4, pe) - 1 - pb) / GL;
+                    c1 = (max(i1, pb) - pb) / CH;
+                    c2 = (min(i4, pe) - 1 - pb) / CH;
                 }
                 const int cmin = __reduce_min_sync(FULL, c1);
                 const int cmax = __reduce_max_sync(FULL, c2);
@@ -318,8 +406,9 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 }
                 sBm[lane * BST + wd] = myword;
                 mycnt += __popc(myword);
+                mywm |= (myword != 0u) ? (1u << wd) : 0u;
             }
-            // -- exclusive prefix over chunks: the item's entries as one flat list
+            // -- exclusive prefix over chunks: the pass's (record, chunk) entries as one flat list
             int incl = mycnt;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
@@ -329,6 +418,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
             const int off = incl - mycnt;
             const int T = __shfl_sync(FULL, incl, 31);
             sOff[lane] = off;
+            sWm[lane] = mywm;
             __syncwarp();
             if (T == 0) continue;
 
@@ -344,53 +434,41 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 if (gg == g) c = 31 - __clz(b);
             }
             int w = 0;
-            uint32_t m = 0;
-            if (worked) {
+            uint32_t m = 0, wm = 0;
+            if (worked) {   // position on entry `start`: skip whole words, then single records
                 int skip = start - sOff[c];
-                m = sBm[c * BST];
-                int pc = __popc(m);
-                while (skip >= pc) {
-                    skip -= pc;
-                    ++w;
+                wm = sWm[c];
+                for (;;) {
+                    w = __ffs(wm) - 1;
+                    wm &= wm - 1;
                     m = sBm[c * BST + w];
-                    pc = __popc(m);
+                    const int pc = __popc(m);
+                    if (skip < pc) break;
+                    skip -= pc;
                 }
                 for (; skip > 0; --skip) m &= m - 1;
             }
-            int bin = pb + c * GL + gl;
-            float om = (bin < nE) ? __ldg(omega + bin) : qnan;
+            int bin0 = pb + c * CH + 2 * gl;
+            f2 om = make_float2((bin0 < nE) ? __ldg(omega + bin0) : qnan, (bin0 + 1 < nE) ? __ldg(omega + bin0 + 1) : qnan);
 
-            float accD[MB], accT[MB];
-#pragma unroll
-            for (int mm = 0; mm < MB; mm++) accD[mm] = accT[mm] = 0.0f;
-
-            auto flush = [&]() {   // this group's registers -> the block's partial histogram
-                if (bin < nE) {
-#pragma unroll
-                    for (int mm = 0; mm < MB; mm++) {
-                        if (m0 + mm < p.norb) {
-                            red_add(partD + (size_t)(m0 + mm) * nE + bin, accD[mm]);
-                            red_add(partT + (size_t)(m0 + mm) * nE + bin, accT[mm]);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int mm = 0; mm < MB; mm++) accD[mm] = accT[mm] = 0.0f;
-            };
+            Acc<MB> acc;
+            acc.zero();
 
             // -- A4-A6: every group walks its share of the list; lanes own bins
 #pragma unroll 1
             for (int step = 0; step < q; ++step) {
                 if (rem > 0) {
-                    while (m == 0) {   // next word / next chunk (uniform within the group)
-                        ++w;
-                        if (w == NWORD) {
-                            flush();
+                    if (m == 0) {   // next non-empty word, possibly of the next chunk (uniform within the group)
+                        while (wm == 0) {
+                            acc.flush(part, bin0, nE, norb, m0, vec4);
                             ++c;
-                            w = 0;
-                            bin += GL;
-                            om = (bin < nE) ? __ldg(omega + bin) : qnan;
+                            bin0 += CH;
+                            om = make_float2((bin0 < nE) ? __ldg(omega + bin0) : qnan,
+                                             (bin0 + 1 < nE) ? __ldg(omega + bin0 + 1) : qnan);
+                            wm = sWm[c];
                         }
+                        w = __ffs(wm) - 1;
+                        wm &= wm - 1;
                         m = sBm[c * BST + w];
                     }
                     const int t = w * 32 + __ffs(m) - 1;
@@ -399,27 +477,13 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
 
                     const float4 es = sEs[t];
                     const uint2 cs = sCs[t];
-                    float wv[4], dw[4];
-                    if (om > es.x && om < es.w) {
-                        corner_weights_in_window(es.x, es.y, es.z, es.w, om, wv, dw);
-                    } else {
-#pragma unroll
-                        for (int l = 0; l < 4; l++) wv[l] = dw[l] = 0.0f;
-                    }
+                    f2 wv[4], dw[4];
+                    corner_weights_x2(es.x, es.y, es.z, es.w, om, wv, dw);
                     const unsigned cc[4] = {cs.x & 0xffffu, cs.x >> 16, cs.y & 0xffffu, cs.y >> 16};
-#pragma unroll
-                    for (int l = 0; l < 4; l++) {
-                        float b[MB];
-                        load_b<MB>(sW + cc[l], b);
-#pragma unroll
-                        for (int mm = 0; mm < MB; mm++) {
-                            accD[mm] = fmaf(b[mm], dw[l], accD[mm]);
-                            accT[mm] = fmaf(b[mm], wv[l], accT[mm]);
-                        }
-                    }
+                    acc.project(sW, cc, wv, dw);
                 }
             }
-            if (worked) flush();
+            if (worked) acc.flush(part, bin0, nE, norb, m0, vec4);
             __syncwarp();   // the next pass rewrites the bitmaps
         }
         __syncwarp();   // the next item rewrites the slice
@@ -435,21 +499,18 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     }
 }
 
-// A7a: sum the block partials in fp64.  out[3][norb][nE]; the step histogram is stored [nE][norb] per block.
+// A7a: sum the block partials in fp64.  out[3][norb][nE] from per-block rows [nE][ D(norb) | T(norb) | S(norb) ].
 __global__ void __launch_bounds__(256) tdos_merge(const float* __restrict__ partial, int nblk, int norb, int nE,
                                                   double* __restrict__ out) {
-    const size_t q = (size_t)norb * nE, n = 3 * q;
+    const size_t n = (size_t)3 * norb * nE;
     for (size_t j = blockIdx.x * (size_t)blockDim.x + threadIdx.x; j < n; j += (size_t)gridDim.x * blockDim.x) {
-        size_t src = j;
-        if (j >= 2 * q) {
-            const size_t r = j - 2 * q, m = r / nE, i = r - m * nE;
-            src = 2 * q + i * norb + m;
-        }
         double s = 0.0;
-        for (int c = 0; c < nblk; c++) s += (double)partial[(size_t)c * n + src];
-        out[j] = s;
+        for (int c = 0; c < nblk; c++) s += (double)partial[(size_t)c * n + j];
+        const size_t i = j / (3 * norb), qm = j - i * (3 * norb);
+        out[qm * nE + i] = s;
     }
 }
+
 // A7b: one block per orbital.  dos = V*D ; nos = V*(T + inclusive prefix over omega of S), fp64 inside.
 __global__ void __launch_bounds__(1024) tdos_finalize(const double* __restrict__ part, int norb, int nE, double V,
                                                       float* __restrict__ dos, float* __restrict__ nos) {

@@ -1,10 +1,18 @@
-// tdos_weights.cuh -- fp32 corner weights of the linear tetrahedron method (device code).
+// tdos_weights.cuh -- fp32 corner weights of the linear tetrahedron method (device code), evaluated for
+// TWO energies at once with Blackwell's packed fp32x2 arithmetic (FFMA2 / FMUL2 / FADD2).
 //
-// PAPER.md Eq. 11-15 (:105-200), written for the GPU: every quotient is formed as a product of
-// ratios bounded by 1 (so nearly degenerate corners cannot overflow, reading G12), the
-// common factor V = V_T/(4 V_G) is left out (applied once, in fp64, by the merge kernel), and the
-// derivative identities  sum_l dw_l = 4 dC  (Eq. 12) /  -4 dC (Eq. 14)  replace the longest
-// expressions (12d, 14f).  Misprints of the paper are read as in DESIGN.md (G1-G5).
+// PAPER.md Eq. 11-15 (:105-200), written for the GPU:
+//   * every quotient is a product of ratios bounded by 1, so nearly degenerate corners cannot overflow
+//     (reading G12); the common factor V = V_T/(4 V_G) is left out (applied once, in fp64, by
+//     the finalize kernel);
+//   * Eq. 12 and Eq. 14 are mirror images (E - E1 <-> E4 - E, corners 1,2,3,4 <-> 4,3,2,1): one code path
+//     ("edge") serves both, its inputs selected per energy;
+//   * Eq. 14's weights are returned as w_j - V (= -C q_j): the constant V of Eq. 14c/e is added by the
+//     caller as a step at the first energy >= E3, together with Eq. 15's;
+//   * the derivative identities  sum_l dw_l = 4 dC  (Eq. 12) / -4 dC (Eq. 14)  replace 12d and 14f;
+//   * misprints of the paper are read as in DESIGN.md (G1-G5).
+// The two energies of a call may fall in different intervals: the edge path and the middle path (Eq. 13)
+// each return exact zeros for the energies they do not serve, and the results are added.
 //
 // This file shares nothing with oracle/ (which restates the same equations literally in fp64).
 #pragma once
@@ -12,82 +20,102 @@
 
 namespace tdos {
 
+typedef float2 f2;
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 dup(float x) { return make_float2(x, x); }
+
 __device__ __forceinline__ float rcp_fast(float x) {
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
 
-// Sorted corner energies e1 <= e2 <= e3 <= e4, energy of interest E with e1 < E < e4.
-// Outputs w[l]/V and (dw[l]/dE)/V for the sorted corners l = 0..3.
-__device__ __forceinline__ void corner_weights_in_window(float e1, float e2, float e3, float e4, float E,
-                                                         float (&w)[4], float (&dw)[4]) {
-    if (E < e2) {
-        // Eq. 12: x = E - E1, r_j = x/E_j1 <= 1, C = r2 r3 r4
-        const float x = E - e1;
-        const float i21 = rcp_fast(e2 - e1), i31 = rcp_fast(e3 - e1), i41 = rcp_fast(e4 - e1);
-        const float r2 = x * i21, r3 = x * i31, r4 = x * i41;
-        const float r23 = r2 * r3;
-        const float C = r23 * r4;                  // 12a
-        const float dC = 3.0f * r23 * i41;         // 12b
-        const float C4 = 4.0f * C;
-        w[1] = C * r2;                             // 12e
-        w[2] = C * r3;
-        w[3] = C * r4;
-        w[0] = fmaf(-C, (r2 + r3) + r4, C4);       // 12c
-        dw[1] = C4 * i21;                          // 12f: dC x/E_j1 + C/E_j1 = 4C/E_j1
-        dw[2] = C4 * i31;
-        dw[3] = C4 * i41;
-        dw[0] = fmaf(4.0f, dC, -((dw[1] + dw[2]) + dw[3]));   // 12d via sum_l dw_l = 4 dC
-    } else if (E < e3) {
-        // Eq. 13
-        const float a = E - e1, b = E - e2, c = e3 - E, d = e4 - E;
-        const float i31 = rcp_fast(e3 - e1), i41 = rcp_fast(e4 - e1);
-        const float i32 = rcp_fast(e3 - e2), i42 = rcp_fast(e4 - e2);
-        const float A31 = a * i31, A41 = a * i41;  // (E-E1)/E31, (E-E1)/E41
-        const float B32 = b * i32, B42 = b * i42;  // (E-E2)/E32, (E-E2)/E42
-        const float C31 = c * i31, C32 = c * i32;  // (E3-E)/E31, (E3-E)/E32
-        const float D41 = d * i41, D42 = d * i42;  // (E4-E)/E41, (E4-E)/E42
-        const float C1 = A31 * A41;                                        // 13a
-        const float dC1 = 2.0f * A31 * i41;                                // 13b
-        const float AB = A31 * B32;
-        const float C2 = A41 * B32 * C31;                                  // 13c
-        const float dC2 = i41 * fmaf(C32 * (a + b), i31, -AB);             // 13d
-        const float BB = B32 * B42;
-        const float C3 = BB * D41;                                         // 13e
-        const float dC3 = B32 * i41 * fmaf(2.0f, D42, -B42);               // 13f
-        const float C12 = C1 + C2, C23 = C2 + C3, C123 = C12 + C3;
-        const float dC12 = dC1 + dC2, dC23 = dC2 + dC3, dC123 = dC12 + dC3;
-        const float P = C12 * C31, Q = C23 * C32, R = C123 * D41, S = C3 * D42;
-        w[0] = (C1 + P) + R;                                               // 13g
-        w[1] = (C123 + Q) + S;                                             // 13i
-        w[2] = (C12 - P) + (C23 - Q);                                      // 13k (G3): (E-E1)/E31 = 1 - (E3-E)/E31
-        w[3] = (C123 - R) + (C3 - S);                                      // 13m
-        const float dP = fmaf(dC12, C31, -C12 * i31);    // d/dE [C12 (E3-E)/E31]
-        const float dQ = fmaf(dC23, C32, -C23 * i32);
-        const float dR = fmaf(dC123, D41, -C123 * i41);
-        const float dS = fmaf(dC3, D42, -C3 * i42);
-        dw[0] = (dC1 + dP) + dR;                                           // 13h
-        dw[1] = (dC123 + dQ) + dS;                                         // 13j
-        dw[2] = (dC12 - dP) + (dC23 - dQ);                                 // 13l (G4)
-        dw[3] = (dC123 - dR) + (dC3 - dS);                                 // 13n
-    } else {
-        // Eq. 14: y = E4 - E, q_j = y/E_4j <= 1, C = q1 q2 q3
-        const float y = e4 - E;
-        const float i41 = rcp_fast(e4 - e1), i42 = rcp_fast(e4 - e2), i43 = rcp_fast(e4 - e3);
-        const float q1 = y * i41, q2 = y * i42, q3 = y * i43;
-        const float q12 = q1 * q2;
-        const float C = q12 * q3;                  // 14a
-        const float mdC = 3.0f * q12 * i43;        // -(14b)
-        const float C4 = 4.0f * C;
-        w[0] = fmaf(-C, q1, 1.0f);                 // 14c
-        w[1] = fmaf(-C, q2, 1.0f);
-        w[2] = fmaf(-C, q3, 1.0f);
-        w[3] = 1.0f - fmaf(-C, (q1 + q2) + q3, C4);    // 14e (G5)
-        dw[0] = C4 * i41;                          // 14d: -dC y/E_4j + C/E_4j = 4C/E_4j
-        dw[1] = C4 * i42;
-        dw[2] = C4 * i43;
-        dw[3] = fmaf(4.0f, mdC, -((dw[0] + dw[1]) + dw[2]));   // 14f via sum_l dw_l = -4 dC
+// Sorted corner energies e1 <= e2 <= e3 <= e4 and two energies E = (Ea, Eb).
+// For each energy with e1 < E < e4:  w[l] = w_l/V (E < e3) or w_l/V - 1 (E >= e3),  dw[l] = (dw_l/dE)/V,
+// for the sorted corners l = 0..3; for an energy outside (e1, e4), or NaN, all eight values are 0.
+__device__ __forceinline__ void corner_weights_x2(float e1, float e2, float e3, float e4, f2 E, f2 (&w)[4], f2 (&dw)[4]) {
+    const bool va = (E.x > e1) && (E.x < e4), vb = (E.y > e1) && (E.y < e4);
+    const bool lo_a = E.x < e2, lo_b = E.y < e2;          // Eq. 12
+    const bool hi_a = E.x >= e3, hi_b = E.y >= e3;        // Eq. 14
+    const bool ed_a = va && (lo_a || hi_a), ed_b = vb && (lo_b || hi_b);
+    const bool mi_a = va && !lo_a && !hi_a, mi_b = vb && !lo_b && !hi_b;   // Eq. 13
+
+    // reciprocals of the six differences E_ij (Eq. 10); a vanishing difference is never USED by a valid
+    // interval (G11), clamping only keeps 0 * (1/0) out of the masked lanes
+    const float tiny = 1e-30f;
+    const float i21 = rcp_fast(fmaxf(e2 - e1, tiny)), i31 = rcp_fast(fmaxf(e3 - e1, tiny));
+    const float i41 = rcp_fast(fmaxf(e4 - e1, tiny)), i32 = rcp_fast(fmaxf(e3 - e2, tiny));
+    const float i42 = rcp_fast(fmaxf(e4 - e2, tiny)), i43 = rcp_fast(fmaxf(e4 - e3, tiny));
+    const f2 I41 = dup(i41);
+    const f2 NEG1 = dup(-1.0f);
+
+#pragma unroll
+    for (int l = 0; l < 4; l++) w[l] = dw[l] = dup(0.0f);
+
+    if (ed_a || ed_b) {
+        // ---- Eq. 12 / Eq. 14: x = E - E1 (or E4 - E); far corners j: r_j = x/E_j1 (or y/E_4j) <= 1;
+        //      C = r r' r'';  w_far = C r_j, dw_far = 4C/E_j1;  w_near = C (4 - sum r), sum_l dw_l = +-4 dC
+        f2 X, I1, I2, SG;
+        X.x = ed_a ? (lo_a ? E.x - e1 : e4 - E.x) : 0.0f;
+        X.y = ed_b ? (lo_b ? E.y - e1 : e4 - E.y) : 0.0f;
+        I1.x = lo_a ? i21 : i42;  I1.y = lo_b ? i21 : i42;     // sorted corner 2
+        I2.x = lo_a ? i31 : i43;  I2.y = lo_b ? i31 : i43;     // sorted corner 3
+        SG.x = lo_a ? 1.0f : -1.0f;  SG.y = lo_b ? 1.0f : -1.0f;   // Eq. 14: w - V = -C q
+        const f2 R1 = mul2(X, I1), R2 = mul2(X, I2), R3 = mul2(X, I41);
+        const f2 R12 = mul2(R1, R2);
+        const f2 C = mul2(R12, R3);                     // 12a / 14a
+        const f2 C4 = mul2(C, dup(4.0f));
+        const f2 Cs = mul2(C, SG);
+        const f2 wF1 = mul2(Cs, R1), wF2 = mul2(Cs, R2), wF3 = mul2(Cs, R3);      // 12e / 14c
+        const f2 dF1 = mul2(C4, I1), dF2 = mul2(C4, I2), dF3 = mul2(C4, I41);     // 12f / 14d
+        const f2 sumR = add2(add2(R1, R2), R3);
+        const f2 wN = fma2(mul2(Cs, NEG1), sumR, mul2(Cs, dup(4.0f)));            // 12c / 14e
+        const f2 dN = fma2(mul2(R12, I41), dup(12.0f), mul2(add2(add2(dF1, dF2), dF3), NEG1));   // 12d / 14f
+        w[1] = wF1; dw[1] = dF1;
+        w[2] = wF2; dw[2] = dF2;
+        // the near corner is corner 1 below E2 and corner 4 above E3; the corner with E_41 is the other one
+        w[0].x = lo_a ? wN.x : wF3.x;   w[0].y = lo_b ? wN.y : wF3.y;
+        w[3].x = lo_a ? wF3.x : wN.x;   w[3].y = lo_b ? wF3.y : wN.y;
+        dw[0].x = lo_a ? dN.x : dF3.x;  dw[0].y = lo_b ? dN.y : dF3.y;
+        dw[3].x = lo_a ? dF3.x : dN.x;  dw[3].y = lo_b ? dF3.y : dN.y;
+    }
+    if (mi_a || mi_b) {
+        // ---- Eq. 13.  For an energy this path does not serve, a = b = 0 makes every term vanish.
+        f2 Es, a;
+        Es.x = mi_a ? E.x : e2;  Es.y = mi_b ? E.y : e2;
+        a.x = mi_a ? Es.x - e1 : 0.0f;  a.y = mi_b ? Es.y - e1 : 0.0f;
+        const f2 b = fma2(dup(e2), NEG1, Es);           // E - E2
+        const f2 c = fma2(Es, NEG1, dup(e3));           // E3 - E
+        const f2 d = fma2(Es, NEG1, dup(e4));           // E4 - E
+        const f2 I31 = dup(i31), I32 = dup(i32), I42 = dup(i42);
+        const f2 A31 = mul2(a, I31), A41 = mul2(a, I41);     // (E-E1)/E31, (E-E1)/E41
+        const f2 B32 = mul2(b, I32), B42 = mul2(b, I42);     // (E-E2)/E32, (E-E2)/E42
+        const f2 C31 = mul2(c, I31), C32 = mul2(c, I32);     // (E3-E)/E31, (E3-E)/E32
+        const f2 D41 = mul2(d, I41), D42 = mul2(d, I42);     // (E4-E)/E41, (E4-E)/E42
+        const f2 C1 = mul2(A31, A41);                                        // 13a
+        const f2 dC1 = mul2(A31, dup(2.0f * i41));                           // 13b
+        const f2 AB = mul2(A31, B32);
+        const f2 C2 = mul2(mul2(A41, B32), C31);                             // 13c
+        const f2 dC2 = mul2(I41, fma2(AB, NEG1, mul2(mul2(C32, add2(a, b)), I31)));   // 13d
+        const f2 C3 = mul2(mul2(B32, B42), D41);                             // 13e
+        const f2 dC3 = mul2(mul2(B32, I41), fma2(B42, NEG1, add2(D42, D42)));   // 13f
+        const f2 C12 = add2(C1, C2), C23 = add2(C2, C3), C123 = add2(C12, C3);
+        const f2 dC12 = add2(dC1, dC2), dC23 = add2(dC2, dC3), dC123 = add2(dC12, dC3);
+        const f2 P = mul2(C12, C31), Q = mul2(C23, C32), R = mul2(C123, D41), S = mul2(C3, D42);
+        const f2 dP = fma2(C12, dup(-i31), mul2(dC12, C31));   // d/dE [C12 (E3-E)/E31]
+        const f2 dQ = fma2(C23, dup(-i32), mul2(dC23, C32));
+        const f2 dR = fma2(C123, dup(-i41), mul2(dC123, D41));
+        const f2 dS = fma2(C3, dup(-i42), mul2(dC3, D42));
+        w[0] = add2(w[0], add2(add2(C1, P), R));                             // 13g
+        w[1] = add2(w[1], add2(add2(C123, Q), S));                           // 13i
+        w[2] = add2(w[2], add2(fma2(P, NEG1, C12), fma2(Q, NEG1, C23)));     // 13k (G3): (E-E1)/E31 = 1 - (E3-E)/E31
+        w[3] = add2(w[3], add2(fma2(R, NEG1, C123), fma2(S, NEG1, C3)));     // 13m
+        dw[0] = add2(dw[0], add2(add2(dC1, dP), dR));                        // 13h
+        dw[1] = add2(dw[1], add2(add2(dC123, dQ), dS));                      // 13j
+        dw[2] = add2(dw[2], add2(fma2(dP, NEG1, dC12), fma2(dQ, NEG1, dC23)));   // 13l (G4)
+        dw[3] = add2(dw[3], add2(fma2(dR, NEG1, dC123), fma2(dS, NEG1, dC3)));   // 13n
     }
 }
 

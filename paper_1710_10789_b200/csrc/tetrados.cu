@@ -51,8 +51,8 @@ int pick_mb(int norb) { return norb <= 1 ? 1 : norb <= 2 ? 2 : norb <= 4 ? 4 : 8
 // TDOS_TILE=<index> selects another one for experiments.
 template <int MB>
 std::vector<Variant> variants_for() {
-    return {make_variant<MB, 4, 4, 4, 8, 12>(), make_variant<MB, 4, 4, 4, 4, 12>(), make_variant<MB, 4, 4, 2, 8, 24>(),
-            make_variant<MB, 4, 4, 2, 4, 24>(), make_variant<MB, 8, 4, 2, 8, 12>()};
+    return {make_variant<MB, 4, 4, 2, 2, 16>(), make_variant<MB, 4, 4, 2, 4, 16>(), make_variant<MB, 4, 4, 4, 2, 12>(),
+            make_variant<MB, 4, 4, 4, 4, 12>(), make_variant<MB, 4, 4, 2, 2, 20>()};
 }
 
 std::vector<Variant> variants(int MB) {
