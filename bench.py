@@ -190,7 +190,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1710_10789_b200 import binding   # raises if libtetrados.so is missing: no CPU fallback
+    from paper_1710_10789_b200 import binding, sharding   # raises if libtetrados.so is missing: no CPU fallback
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
@@ -218,7 +218,7 @@ def main():
     dos = torch.zeros((norb, nE), device=dev)
     nos = torch.zeros((norb, nE), device=dev)
     part = torch.zeros((3, norb, nE), dtype=torch.float64, device=dev)
-    z_lo, z_hi = (N3 * rank) // world, (N3 * (rank + 1)) // world
+    z_lo, z_hi = sharding.z_slab(rank, world, N3)
     plan = binding.Plan(cfg.nk, nb, norb, nE, device=local_rank)
 
     def step():

@@ -131,7 +131,9 @@ int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, f
  * tdos_last_counters: exact work counters of the last tetra_dos / tetra_dos_partial call, counted by
  *   the main kernel: cnt[0] = n_tb = (tetrahedron, band) pairs processed, cnt[1] = n_eval = number of
  *   (tetrahedron, band, omega_i) with E1 < omega_i < E4, i.e. evaluations of Eq. 12-14 the method
- *   needs.  Synchronises the call's stream.
+ *   needs; cnt[2] = how many of them fall in the middle interval E2 <= omega_i < E3
+ *   (Eq. 13; -1 if the kernel generation does not count it), cnt[3] = main kernel generation (3 or 4).
+ *   Synchronises the call's stream.
  * tdos_kernel_ms: mean device time of the main kernel and of the merge+finalize kernels over the
  *   last `ncalls` (1..64) device-mode tetra_dos calls on this plan, from CUDA events the library records
  *   on each call's stream around its own launches (waits for those calls to finish).
@@ -140,7 +142,7 @@ int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, f
  *   returns the achieved FP32 rate in TFLOP/s (2 flops per FMA lane) in *tflops.
  */
 int tdos_plan_info(const tdos_plan* p, long long what[8]);
-int tdos_last_counters(tdos_plan* p, long long cnt[2]);
+int tdos_last_counters(tdos_plan* p, long long cnt[4]);
 int tdos_kernel_ms(tdos_plan* p, int ncalls, float* main_ms, float* merge_ms);
 int tdos_last_kernel_ms(tdos_plan* p, float* main_ms, float* merge_ms);
 int tdos_fp32_fma_probe(tdos_plan* p, int packed, double* tflops);

@@ -132,9 +132,9 @@ class Plan:
         return {"grid": w[0], "threads": w[1], "smem": w[2], "items": w[3], "launches": w[4], "tile": (w[5], w[6], w[7])}
 
     def last_counters(self) -> dict:
-        w = (C.c_longlong * 2)()
+        w = (C.c_longlong * 4)()
         _check(load().tdos_last_counters(self._h, w), "tdos_last_counters")
-        return {"n_tb": w[0], "n_eval": w[1]}
+        return {"n_tb": w[0], "n_eval": w[1], "n_eval_mid": w[2], "kernel": w[3]}
 
     def kernel_ms(self, ncalls: int = 1):
         """(main kernel ms, merge+finalize ms), mean over the last `ncalls` device-mode calls."""

@@ -13,10 +13,14 @@
 #include <vector>
 
 #include "tdos_kernels.cuh"
+#include "tdos_main4.cuh"
 
 namespace {
 
 thread_local char g_cuda_err[256] = "";
+
+// host mode: bytes of E + W per staged z-slab (copy/compute overlap granularity)
+constexpr size_t kSlabBytes = (size_t)64 << 20;
 
 int cuda_fail(cudaError_t e, const char* what) {
     snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
@@ -29,14 +33,31 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
+using tdos::Main4Params;
 using tdos::MainParams;
 typedef void (*main_kernel_t)(const MainParams);
+typedef void (*main4_kernel_t)(const Main4Params);
 
 struct Variant {
-    main_kernel_t fn;
+    main_kernel_t fn;      // v3 kernel (default), or null
     int MB, TX, TY, TZ, GL, NWARP;
     size_t smem;
+    main4_kernel_t fn4 = nullptr;   // v4 kernel (TDOS_KERNEL=4, experimental: DESIGN.md 4.2)
+    int BX = 0;                     // v4: tiles per batch
 };
+
+template <int TX, int TY, int TZ, int NWARP>
+Variant make_variant4() {
+    Variant v{nullptr, 8, TX, TY, TZ, 2, NWARP, (size_t)NWARP * tdos::Cfg4<TX, TY, TZ>::bytes};
+    v.fn4 = tdos::tdos_main4<TX, TY, TZ, NWARP>;
+    v.BX = tdos::Cfg4<TX, TY, TZ>::BX;
+    return v;
+}
+
+// v4 configurations compiled in (TDOS_TILE=<index> selects another one for experiments)
+std::vector<Variant> variants4() {
+    return {make_variant4<2, 2, 2, 8>(), make_variant4<4, 2, 1, 8>(), make_variant4<2, 2, 1, 12>()};
+}
 
 template <int MB, int TX, int TY, int TZ, int GL, int NWARP>
 Variant make_variant() {
@@ -87,6 +108,8 @@ struct tdos_plan {
     cudaStream_t main = nullptr;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // [3] and [2] bracket the FMA probe
     // ring of event triples (before main kernel, after it, after merge+finalize), one per tetra_dos call
+    static constexpr int kMaxSlabs = 32;
+    cudaEvent_t cp_ev[kMaxSlabs] = {};   // host mode: slab s has arrived on the device
     static constexpr int kRing = 64;
     cudaEvent_t ring[kRing][3] = {};
     long long n_timed_calls = 0;   // tetra_dos (device path) calls since plan creation
@@ -129,6 +152,8 @@ int tdos_plan_destroy(tdos_plan* p) {
     cudaFree(p->dNos);
     for (auto& e : p->ev)
         if (e) cudaEventDestroy(e);
+    for (auto& e : p->cp_ev)
+        if (e) cudaEventDestroy(e);
     for (auto& tr : p->ring)
         for (auto& e : tr)
             if (e) cudaEventDestroy(e);
@@ -156,15 +181,17 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     p->nE_max = nE_max;
     p->num_sms = prop.multiProcessorCount;
 
-    std::vector<Variant> vs = variants(pick_mb(norb));
+    const char* kv = getenv("TDOS_KERNEL");
+    std::vector<Variant> vs = (kv && atoi(kv) == 4) ? variants4() : variants(pick_mb(norb));
     int sel = 0;
     if (const char* s = getenv("TDOS_TILE")) sel = atoi(s);
     if (sel < 0 || sel >= (int)vs.size()) sel = 0;
     p->var = vs[sel];
 
-    cudaError_t e = cudaFuncSetAttribute(p->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->var.smem);
+    const void* kfn = p->var.fn4 ? (const void*)p->var.fn4 : (const void*)p->var.fn;
+    cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->var.smem);
     if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->blocks_per_sm, p->var.fn, p->var.NWARP * 32, p->var.smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->blocks_per_sm, kfn, p->var.NWARP * 32, p->var.smem);
     if (e != cudaSuccess || p->blocks_per_sm < 1) {
         int rc = (e != cudaSuccess) ? cuda_fail(e, "kernel setup") : TDOS_ECUDA;
         delete p;
@@ -179,7 +206,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     const size_t hist = (size_t)3 * norb * nE_max;
     if (cudaMalloc(&p->partial, hist * p->grid * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&p->part64, hist * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&p->counters, 2 * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaMalloc(&p->counters, 4 * sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError();
         tdos_plan_destroy(p);
         return TDOS_ENOMEM;
@@ -215,9 +242,10 @@ static int check_common(const tdos_plan* p, const float* E, const float* W, int 
     return TDOS_OK;
 }
 
-// enqueue: zero partials, main kernel, merge into part64_out (device fp64 [3][norb][nE])
-static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
-                           int z_lo, int z_hi, double* part_out, cudaStream_t st) {
+// enqueue the main kernel for the cube slab [z_lo, z_hi); `first` also clears the block partials and the
+// work counters (a call may cover the grid with several slab launches that accumulate into the same partials)
+static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+                        int z_lo, int z_hi, bool first, cudaStream_t st) {
     const Variant& v = p->var;
     const long long nkt = (long long)p->nk[0] * p->nk[1] * p->nk[2];
     MainParams mp{};
@@ -245,30 +273,67 @@ static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int lay
     mp.partial = p->partial;
     mp.counters = p->counters;
 
+    Main4Params m4{};
+    long long work = items;   // independent units the warps draw: items (v3) or batches of tiles (v4)
+    if (v.fn4) {
+        m4.nbx = (mp.ntx + v.BX - 1) / v.BX;
+        work = (long long)m4.nbx * mp.nty * mp.ntz * p->nb * mp.nmb;
+        m4.n_batches = (int)work;
+        m4.next_batch = reinterpret_cast<unsigned int*>(p->counters + 3);
+    }
     const size_t hist = (size_t)3 * p->norb * nE;
-    const long long blocks_needed = (items + v.NWARP - 1) / v.NWARP;
-    const int grid = (int)((blocks_needed < p->grid) ? (blocks_needed > 0 ? blocks_needed : 1) : p->grid);
-    CK(cudaMemsetAsync(p->partial, 0, hist * grid * sizeof(float), st));
-    CK(cudaMemsetAsync(p->counters, 0, 2 * sizeof(unsigned long long), st));
-    CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
-    v.fn<<<grid, v.NWARP * 32, v.smem, st>>>(mp);
-    CK(cudaGetLastError());
-    CK(cudaEventRecord(p->ring[p->cur_slot][1], st));
-    const int mblocks = (int)((hist + 255) / 256);
-    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, grid, p->norb, nE, part_out);
-    CK(cudaGetLastError());
-    p->last_items = items;
-    p->last_launches = 2;
+    if (first) {
+        CK(cudaMemsetAsync(p->partial, 0, hist * p->grid * sizeof(float), st));
+        CK(cudaMemsetAsync(p->counters, 0, 4 * sizeof(unsigned long long), st));
+        p->last_items = 0;
+        p->last_launches = 0;
+    } else if (v.fn4) {
+        CK(cudaMemsetAsync(p->counters + 3, 0, sizeof(unsigned long long), st));
+    }
+    if (work > 0) {
+        const long long blocks_needed = (work + v.NWARP - 1) / v.NWARP;
+        const int grid = (int)((blocks_needed < p->grid) ? blocks_needed : p->grid);
+        if (v.fn4) {
+            m4.b = mp;
+            v.fn4<<<grid, v.NWARP * 32, v.smem, st>>>(m4);
+        } else {
+            v.fn<<<grid, v.NWARP * 32, v.smem, st>>>(mp);
+        }
+        CK(cudaGetLastError());
+        p->last_launches += 1;
+    }
+    p->last_items += items;
     p->last_stream = st;
     p->last_stream_valid = true;
     p->timed = false;
     return TDOS_OK;
 }
 
+// fp64 sum of the block partials -> part_out (device fp64 [3][norb][nE])
+static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st) {
+    const size_t hist = (size_t)3 * p->norb * nE;
+    const int mblocks = (int)((hist + 255) / 256);
+    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->grid, p->norb, nE, part_out);
+    CK(cudaGetLastError());
+    p->last_launches += 1;
+    return TDOS_OK;
+}
+
+// zero partials, main kernel over [z_lo, z_hi), merge into part_out; events around the main kernel
+static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+                           int z_lo, int z_hi, double* part_out, cudaStream_t st) {
+    CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
+    int rc = enqueue_main(p, E, W, layout, omega, nE, z_lo, z_hi, true, st);
+    if (rc) return rc;
+    CK(cudaEventRecord(p->ring[p->cur_slot][1], st));
+    return enqueue_merge(p, nE, part_out, st);
+}
+
 static int enqueue_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos, cudaStream_t st) {
     const double V = 1.0 / (24.0 * (double)p->nk[0] * (double)p->nk[1] * (double)p->nk[2]);
     tdos::tdos_finalize<<<p->norb, 1024, 0, st>>>(part, p->norb, nE, V, dos, nos);
     CK(cudaGetLastError());
+    p->last_launches += 1;
     return TDOS_OK;
 }
 
@@ -302,7 +367,6 @@ static int run_device(tdos_plan* p, const float* E, const float* W, int layout, 
     if (rc) return rc;
     CK(cudaEventRecord(p->ring[p->cur_slot][2], st));
     p->n_timed_calls++;
-    p->last_launches = 3;
     p->timed = true;
     return TDOS_OK;
 }
@@ -332,12 +396,55 @@ int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const fl
             return TDOS_ENOMEM;
         }
     }
-    cudaStream_t st = p->main;
+    // A0 ("called from a CPU code"): the grid is cut into z-slabs; slab s is copied on the
+    // side stream while the main kernel works on slab s-1.  Copy s brings the planes (z_s, z_{s+1}] (copy 0
+    // also plane 0), so the cubes of slab s -- which read planes z_s .. z_{s+1}, the last one wrapping to
+    // plane 0 -- need copies 0..s only.
+    cudaStream_t st = p->main, cp = p->side;
+    const int N3 = p->nk[2];
+    const size_t plane = (size_t)p->nk[0] * p->nk[1];
+    const size_t total = nkt * p->nb * (1 + (W ? (size_t)p->norb : 0)) * sizeof(float);
+    int nslab = (int)((total + kSlabBytes - 1) / kSlabBytes);
+    if (nslab > tdos_plan::kMaxSlabs) nslab = tdos_plan::kMaxSlabs;
+    if (nslab > N3) nslab = N3;
+    if (nslab < 1) nslab = 1;
+    for (int i = 0; i < nslab; i++)
+        if (!p->cp_ev[i]) CK(cudaEventCreateWithFlags(&p->cp_ev[i], cudaEventDisableTiming));
     CK(cudaMemcpyAsync(p->dOm, omega, (size_t)nE * sizeof(float), cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(p->dE, E, nkt * p->nb * sizeof(float), cudaMemcpyHostToDevice, st));
-    if (W) CK(cudaMemcpyAsync(p->dW, W, nkt * p->nb * p->norb * sizeof(float), cudaMemcpyHostToDevice, st));
-    rc = run_device(p, p->dE, W ? p->dW : nullptr, layout, p->dOm, nE, p->dDos, p->dNos, st);
+    p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
+    CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
+    for (int sidx = 0; sidx < nslab; sidx++) {
+        const int z_lo = (int)((long long)N3 * sidx / nslab), z_hi = (int)((long long)N3 * (sidx + 1) / nslab);
+        const int c_lo = sidx == 0 ? 0 : z_lo + 1, c_hi = (z_hi + 1 < N3) ? z_hi + 1 : N3;
+        if (c_hi > c_lo) {
+            const size_t k0 = (size_t)c_lo * plane, nk_s = (size_t)(c_hi - c_lo) * plane;
+            if (layout == TDOS_AOS) {
+                const size_t se = (size_t)p->nb, sw = (size_t)p->nb * p->norb;
+                CK(cudaMemcpyAsync(p->dE + k0 * se, E + k0 * se, nk_s * se * sizeof(float), cudaMemcpyHostToDevice, cp));
+                if (W)
+                    CK(cudaMemcpyAsync(p->dW + k0 * sw, W + k0 * sw, nk_s * sw * sizeof(float), cudaMemcpyHostToDevice, cp));
+            } else {   // SoA: one strided copy of the slab's k-range for every band (and orbital)
+                const size_t pitch = nkt * sizeof(float);
+                CK(cudaMemcpy2DAsync(p->dE + k0, pitch, E + k0, pitch, nk_s * sizeof(float), (size_t)p->nb,
+                                     cudaMemcpyHostToDevice, cp));
+                if (W)
+                    CK(cudaMemcpy2DAsync(p->dW + k0, pitch, W + k0, pitch, nk_s * sizeof(float),
+                                         (size_t)p->nb * p->norb, cudaMemcpyHostToDevice, cp));
+            }
+        }
+        CK(cudaEventRecord(p->cp_ev[sidx], cp));
+        CK(cudaStreamWaitEvent(st, p->cp_ev[sidx], 0));
+        rc = enqueue_main(p, p->dE, W ? p->dW : nullptr, layout, p->dOm, nE, z_lo, z_hi, sidx == 0, st);
+        if (rc) return rc;
+    }
+    CK(cudaEventRecord(p->ring[p->cur_slot][1], st));
+    rc = enqueue_merge(p, nE, p->part64, st);
     if (rc) return rc;
+    rc = enqueue_finalize(p, p->part64, nE, p->dDos, p->dNos, st);
+    if (rc) return rc;
+    CK(cudaEventRecord(p->ring[p->cur_slot][2], st));
+    p->n_timed_calls++;
+    p->timed = true;
     CK(cudaMemcpyAsync(dos, p->dDos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
     if (nos) CK(cudaMemcpyAsync(nos, p->dNos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -381,14 +488,16 @@ int tdos_plan_info(const tdos_plan* p, long long what[8]) {
     return TDOS_OK;
 }
 
-int tdos_last_counters(tdos_plan* p, long long cnt[2]) {
+int tdos_last_counters(tdos_plan* p, long long cnt[4]) {
     if (!p || !cnt || !p->last_stream_valid) return TDOS_EINVAL;
     CK(cudaSetDevice(p->device));
     CK(cudaStreamSynchronize(p->last_stream));
-    unsigned long long h[2];
+    unsigned long long h[3];
     CK(cudaMemcpy(h, p->counters, sizeof(h), cudaMemcpyDeviceToHost));
     cnt[0] = (long long)h[0];
     cnt[1] = (long long)h[1];
+    cnt[2] = p->var.fn4 ? (long long)h[2] : -1;
+    cnt[3] = p->var.fn4 ? 4 : 3;
     return TDOS_OK;
 }
 

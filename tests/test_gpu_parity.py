@@ -194,3 +194,56 @@ def test_tetra_dos_simple_host_oneshot():
     nos = np.zeros((8, nE), dtype=np.float32)
     binding.tetra_dos_simple(E, W, 10, 8, 8, -6.0, 4.0, nE, dos, nos)
     assert_parity(ref, dos, nos, "simple")
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times (default plan, AoS,
+# device-resident; config 5 also through the HOST path it is defined on).  The windowed oracle
+# (pinned against the literal one by test_P9_invariances_and_variants) computes every output here,
+# so the comparison is element by element, not sampled; the kernel's exact work counters must equal
+# the oracle's, and the sum rule N_m(omega_max) = (1/nk) sum_k sum_n W (P6) must hold at full size.
+def _full_config(name, cache_dir, host=False):
+    import torch
+    cfg = wl.CONFIGS[name]
+    E, W, om = wl.make_inputs(cfg, cache_dir)
+    ref = oracle.tetra_dos(E, W, cfg.nk, om, windowed=True, nthreads=_threads())
+    with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
+        dos, nos = run_gpu(E, W, cfg.nk, om, plan=plan,
+                           memspace=binding.TDOS_HOST if host else binding.TDOS_DEVICE)
+        cnt = plan.last_counters()
+    d, en = assert_parity(ref, dos, nos, name)
+    assert cnt["n_tb"] == ref["n_tb"] == 6 * int(np.prod(cfg.nk)) * cfg.nb
+    assert cnt["n_eval"] == ref["n_eval"]
+    total = W.astype(np.float64).sum(axis=(0, 1)) / np.prod(cfg.nk)
+    assert np.allclose(nos[:, -1], total, rtol=2e-6)
+    print("%s%s dDOS %.2e dN %.2e n_eval %d" % (name, " (host)" if host else "", d, en, cnt["n_eval"]))
+    torch.cuda.empty_cache()
+
+
+def test_cfg3_full_size(cache_dir):
+    _full_config("cfg3", cache_dir)
+
+
+def test_cfg4_full_size_headline(cache_dir):
+    _full_config("cfg4", cache_dir)
+
+
+def test_cfg5_full_size_host_inputs(cache_dir):
+    _full_config("cfg5", cache_dir, host=True)
+
+
+def test_experimental_kernel_generation_4(monkeypatch):
+    """TDOS_KERNEL=4 selects the hoisted-coefficient kernel: same results."""
+    monkeypatch.setenv("TDOS_KERNEL", "4")
+    for nk, nb, norb, nE in (((9, 10, 11), 2, 8, 1000), ((5, 3, 7), 3, 5, 333), ((6, 6, 6), 4, 12, 257)):
+        E, W = wl.random_bands(nk, nb, norb, seed=100 + nk[0] + nE)
+        om = wl.omega_grid(-1.2, 1.3, nE)
+        ref = oracle.tetra_dos(E, W, nk, om)
+        with binding.Plan(nk, nb, norb, nE) as plan:
+            dos, nos = run_gpu(E, W, nk, om, plan=plan)
+            assert plan.last_counters()["kernel"] == 4
+        assert_parity(ref, dos, nos, "kernel 4 %s" % (nk,))
+    E, W = wl.tb8_bands((12, 12, 12), threads=1)
+    om = wl.omega_grid(-6.0, 4.0, 900)
+    ref = oracle.tetra_dos(E, W, (12, 12, 12), om, nthreads=_threads())
+    dos, nos = run_gpu(E, W, (12, 12, 12), om)
+    assert_parity(ref, dos, nos, "kernel 4 tb8")
