@@ -38,6 +38,7 @@ struct MainParams {
     long long sEk, sEn;          // E[ik*sEk + n*sEn]
     long long sWk, sWn, sWm;     // W[ik*sWk + n*sWn + m*sWm]
     int N1, N2, N3, nb, norb, nE;
+    int nEp;                     // rows per block in `partial` (nE, or nE rounded up to 4 for tdos_main5)
     int z_lo, z_hi;              // cube slab [z_lo, z_hi)
     int ntx, nty, ntz;           // tiles per direction (z over the slab)
     int nmb;                     // orbital blocks of MB
@@ -500,12 +501,12 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
 }
 
 // A7a: sum the block partials in fp64.  out[3][norb][nE] from per-block rows [nE][ D(norb) | T(norb) | S(norb) ].
-__global__ void __launch_bounds__(256) tdos_merge(const float* __restrict__ partial, int nblk, int norb, int nE,
+__global__ void __launch_bounds__(256) tdos_merge(const float* __restrict__ partial, int nblk, int norb, int nE, int nEp,
                                                   double* __restrict__ out) {
-    const size_t n = (size_t)3 * norb * nE;
+    const size_t n = (size_t)3 * norb * nE, bstride = (size_t)3 * norb * nEp;
     for (size_t j = blockIdx.x * (size_t)blockDim.x + threadIdx.x; j < n; j += (size_t)gridDim.x * blockDim.x) {
         double s = 0.0;
-        for (int c = 0; c < nblk; c++) s += (double)partial[(size_t)c * n + j];
+        for (int c = 0; c < nblk; c++) s += (double)partial[(size_t)c * bstride + j];
         const size_t i = j / (3 * norb), qm = j - i * (3 * norb);
         out[qm * nE + i] = s;
     }

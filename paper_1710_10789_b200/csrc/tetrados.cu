@@ -14,6 +14,7 @@
 
 #include "tdos_kernels.cuh"
 #include "tdos_main4.cuh"
+#include "tdos_main5.cuh"
 
 namespace {
 
@@ -44,13 +45,28 @@ struct Variant {
     size_t smem;
     main4_kernel_t fn4 = nullptr;   // v4 kernel (TDOS_KERNEL=4, experimental: DESIGN.md 4.2)
     int BX = 0;                     // v4: tiles per batch
+    int gen = 3;                    // main kernel generation: 3, 4 or 5
 };
+
+template <int TX, int TY, int TZ, int NWARP>
+Variant make_variant5() {
+    Variant v{tdos::tdos_main5<TX, TY, TZ, NWARP>, 8, TX, TY, TZ, 2, NWARP, (size_t)NWARP * tdos::Cfg5<TX, TY, TZ>::bytes};
+    v.gen = 5;
+    return v;
+}
+
+// v5 configurations compiled in (TDOS_TILE=<index> selects another one for experiments)
+std::vector<Variant> variants5() {
+    return {make_variant5<4, 4, 2, 16>(), make_variant5<4, 4, 2, 12>(), make_variant5<4, 4, 1, 16>(),
+            make_variant5<4, 4, 1, 20>(), make_variant5<4, 2, 2, 20>()};
+}
 
 template <int TX, int TY, int TZ, int NWARP>
 Variant make_variant4() {
     Variant v{nullptr, 8, TX, TY, TZ, 2, NWARP, (size_t)NWARP * tdos::Cfg4<TX, TY, TZ>::bytes};
     v.fn4 = tdos::tdos_main4<TX, TY, TZ, NWARP>;
     v.BX = tdos::Cfg4<TX, TY, TZ>::BX;
+    v.gen = 4;
     return v;
 }
 
@@ -182,7 +198,10 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     p->num_sms = prop.multiProcessorCount;
 
     const char* kv = getenv("TDOS_KERNEL");
-    std::vector<Variant> vs = (kv && atoi(kv) == 4) ? variants4() : variants(pick_mb(norb));
+    // generation 5 needs blocks of 8 orbitals to pay off; narrower problems use generation 3
+    int gen = kv ? atoi(kv) : 5;
+    if (gen == 5 && (norb < 5 || norb % 4 != 0)) gen = 3;   // tdos_main5: blocks of 8 orbitals, 16-byte vector reductions
+    std::vector<Variant> vs = gen == 4 ? variants4() : gen == 5 ? variants5() : variants(pick_mb(norb));
     int sel = 0;
     if (const char* s = getenv("TDOS_TILE")) sel = atoi(s);
     if (sel < 0 || sel >= (int)vs.size()) sel = 0;
@@ -203,7 +222,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     }
     p->grid = p->num_sms * p->blocks_per_sm;
 
-    const size_t hist = (size_t)3 * norb * nE_max;
+    const size_t hist = (size_t)3 * norb * ((size_t)nE_max + 3);
     if (cudaMalloc(&p->partial, hist * p->grid * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&p->part64, hist * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&p->counters, 4 * sizeof(unsigned long long)) != cudaSuccess) {
@@ -242,6 +261,9 @@ static int check_common(const tdos_plan* p, const float* E, const float* W, int 
     return TDOS_OK;
 }
 
+// rows of one block's partial histogram: generation 5 flushes whole chunks of 4 bins
+static int rows_per_block(const tdos_plan* p, int nE) { return p->var.gen == 5 ? (nE + 3) & ~3 : nE; }
+
 // enqueue the main kernel for the cube slab [z_lo, z_hi); `first` also clears the block partials and the
 // work counters (a call may cover the grid with several slab launches that accumulate into the same partials)
 static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
@@ -261,6 +283,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     }
     mp.N1 = p->nk[0]; mp.N2 = p->nk[1]; mp.N3 = p->nk[2];
     mp.nb = p->nb; mp.norb = p->norb; mp.nE = nE;
+    mp.nEp = rows_per_block(p, nE);
     mp.z_lo = z_lo; mp.z_hi = z_hi;
     mp.ntx = (p->nk[0] + v.TX - 1) / v.TX;
     mp.nty = (p->nk[1] + v.TY - 1) / v.TY;
@@ -281,7 +304,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         m4.n_batches = (int)work;
         m4.next_batch = reinterpret_cast<unsigned int*>(p->counters + 3);
     }
-    const size_t hist = (size_t)3 * p->norb * nE;
+    const size_t hist = (size_t)3 * p->norb * mp.nEp;
     if (first) {
         CK(cudaMemsetAsync(p->partial, 0, hist * p->grid * sizeof(float), st));
         CK(cudaMemsetAsync(p->counters, 0, 4 * sizeof(unsigned long long), st));
@@ -313,7 +336,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
 static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st) {
     const size_t hist = (size_t)3 * p->norb * nE;
     const int mblocks = (int)((hist + 255) / 256);
-    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->grid, p->norb, nE, part_out);
+    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->grid, p->norb, nE, rows_per_block(p, nE), part_out);
     CK(cudaGetLastError());
     p->last_launches += 1;
     return TDOS_OK;
@@ -496,8 +519,8 @@ int tdos_last_counters(tdos_plan* p, long long cnt[4]) {
     CK(cudaMemcpy(h, p->counters, sizeof(h), cudaMemcpyDeviceToHost));
     cnt[0] = (long long)h[0];
     cnt[1] = (long long)h[1];
-    cnt[2] = p->var.fn4 ? (long long)h[2] : -1;
-    cnt[3] = p->var.fn4 ? 4 : 3;
+    cnt[2] = p->var.gen >= 4 ? (long long)h[2] : -1;
+    cnt[3] = p->var.gen;
     return TDOS_OK;
 }
 

@@ -247,3 +247,8 @@ def test_experimental_kernel_generation_4(monkeypatch):
     ref = oracle.tetra_dos(E, W, (12, 12, 12), om, nthreads=_threads())
     dos, nos = run_gpu(E, W, (12, 12, 12), om)
     assert_parity(ref, dos, nos, "kernel 4 tb8")
+
+
+def test_paper_shaped_anisotropic_grid(cache_dir):
+    """60 x 60 x 10 k-points, 8 bands, 1024 energies (the shapes of Table II's last row)."""
+    _full_config("paper60", cache_dir)
