@@ -53,12 +53,19 @@ struct Cfg5 {
     static constexpr size_t bytes = off_un + (sz_setup > sz_walk ? sz_setup : sz_walk);
 };
 
+// a packed pair of zeros in one 64-bit move (keeps ptxas from materialising 32 scalar moves per flush)
+__device__ __forceinline__ f2 zero2() {
+    f2 r;
+    asm volatile("{ .reg .b64 t; mov.b64 t, 0; mov.b64 {%0, %1}, t; }" : "=f"(r.x), "=f"(r.y));
+    return r;
+}
+
 // ---- low/high phase: lane = 4 bins x 4 orbitals x {D, T}
 struct AccE {
     f2 D[4][2], T[4][2];
     __device__ __forceinline__ void zero() {
 #pragma unroll
-        for (int b = 0; b < 4; b++) D[b][0] = D[b][1] = T[b][0] = T[b][1] = make_float2(0.f, 0.f);
+        for (int b = 0; b < 4; b++) { D[b][0] = zero2(); D[b][1] = zero2(); T[b][0] = zero2(); T[b][1] = zero2(); }
     }
     // rows [bin][ D(norb) | T(norb) | S(norb) ] of the block's partial histogram (padded to a multiple of 4 bins,
     // norb % 4 == 0); row = first row of the chunk, at this lane's orbitals
@@ -79,7 +86,7 @@ struct AccM {
 #pragma unroll
         for (int b = 0; b < 2; b++)
 #pragma unroll
-            for (int j = 0; j < 4; j++) D[b][j] = T[b][j] = make_float2(0.f, 0.f);
+            for (int j = 0; j < 4; j++) { D[b][j] = zero2(); T[b][j] = zero2(); }
     }
     // acc += b[l][:] * (dw[l], w[l]) for the 4 sorted corners; w, dw packed along the two bins
     __device__ __forceinline__ void project(const float* __restrict__ sW, const unsigned (&cc)[4], const f2 (&w)[4],
@@ -365,7 +372,9 @@ __device__ __forceinline__ void walk5(unsigned char* __restrict__ base, float* _
     __syncwarp();
 }
 
-template <int TX, int TY, int TZ, int NWARP>
+// NORB = 8: the number of orbitals is fixed at compile time (all histogram offsets become immediates); 0: any
+// multiple of 4
+template <int TX, int TY, int TZ, int NWARP, int NORB>
 __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) {
     using C = Cfg5<TX, TY, TZ>;
     constexpr int PX = C::PX, PY = C::PY, PK = C::PK, NC = C::NC, NTB = C::NTB, WST = C::WST, MB = C::MB;
@@ -380,7 +389,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
     float* sW = reinterpret_cast<float*>(base + C::off_w);
     float* sE = reinterpret_cast<float*>(base + C::off_un);
 
-    const int nE = p.nE, norb = p.norb;
+    const int nE = p.nE, norb = NORB ? NORB : p.norb;
     const float* __restrict__ omega = p.omega;
     const float om0 = __ldg(omega);
     float inv_dom = 0.0f;

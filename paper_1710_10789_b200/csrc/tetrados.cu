@@ -48,17 +48,19 @@ struct Variant {
     int gen = 3;                    // main kernel generation: 3, 4 or 5
 };
 
-template <int TX, int TY, int TZ, int NWARP>
+template <int TX, int TY, int TZ, int NWARP, int NORB>
 Variant make_variant5() {
-    Variant v{tdos::tdos_main5<TX, TY, TZ, NWARP>, 8, TX, TY, TZ, 2, NWARP, (size_t)NWARP * tdos::Cfg5<TX, TY, TZ>::bytes};
+    Variant v{tdos::tdos_main5<TX, TY, TZ, NWARP, NORB>, 8, TX, TY, TZ, 2, NWARP,
+              (size_t)NWARP * tdos::Cfg5<TX, TY, TZ>::bytes};
     v.gen = 5;
     return v;
 }
 
-// v5 configurations compiled in (TDOS_TILE=<index> selects another one for experiments)
+// v5 configurations compiled in (TDOS_TILE=<index> selects another one for experiments); norb == 8 has its own
+// instantiation with compile-time histogram offsets
+template <int NORB>
 std::vector<Variant> variants5() {
-    return {make_variant5<4, 4, 2, 16>(), make_variant5<4, 4, 2, 12>(), make_variant5<4, 4, 1, 16>(),
-            make_variant5<4, 4, 1, 20>(), make_variant5<4, 2, 2, 20>()};
+    return {make_variant5<4, 4, 2, 16, NORB>(), make_variant5<4, 4, 2, 12, NORB>(), make_variant5<4, 4, 1, 16, NORB>()};
 }
 
 template <int TX, int TY, int TZ, int NWARP>
@@ -201,7 +203,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     // generation 5 needs blocks of 8 orbitals to pay off; narrower problems use generation 3
     int gen = kv ? atoi(kv) : 5;
     if (gen == 5 && (norb < 5 || norb % 4 != 0)) gen = 3;   // tdos_main5: blocks of 8 orbitals, 16-byte vector reductions
-    std::vector<Variant> vs = gen == 4 ? variants4() : gen == 5 ? variants5() : variants(pick_mb(norb));
+    std::vector<Variant> vs = gen == 4 ? variants4() : gen == 5 ? (norb == 8 ? variants5<8>() : variants5<0>()) : variants(pick_mb(norb));
     int sel = 0;
     if (const char* s = getenv("TDOS_TILE")) sel = atoi(s);
     if (sel < 0 || sel >= (int)vs.size()) sel = 0;
