@@ -36,11 +36,22 @@ if ROOT not in sys.path:
 
 from paper_1710_10789_b200 import workloads as wl  # noqa: E402  (input generators only)
 
-# Algorithmic flop model: per in-window evaluation
-# F_eval = 40 + 18*norb (weights of Eq. 12-14 case-averaged + 2*4*norb FMAs + 2*norb adds), per
-# (tetrahedron, band) F_tb = 40 + 5*norb (sort, differences, reciprocals, Eq.-15 sum).
+# Algorithmic flop models.
+# Paper formulation (Eq. 12-14 weights per energy, then the orbital loop): per in-window evaluation
+# F_eval = 40 + 18*norb (weights case-averaged + 2*4*norb FMAs + 2*norb adds), per (tetrahedron, band)
+# F_tb = 40 + 5*norb (sort, differences, reciprocals, Eq.-15 sum).
 def flops_alg(n_eval: int, n_tb: int, norb: int) -> float:
     return float(n_eval) * (40 + 18 * norb) + float(n_tb) * (40 + 5 * norb)
+
+
+# Formulation of main kernel generation 5 (recounted, as SURVEY.md 8(d) requires when the formulation changes:
+# algorithmic flops may not exceed executed flops).  Low/high evaluations (Eq. 12/14 with H, J hoisted):
+# T and D each 2 FMAs per orbital + 8 flops for the powers of s -> 8*norb + 8.  Mid evaluations (Eq. 13):
+# ~70 flops for the eight weights + 2*(2*4*norb) for the projection (the accumulation rides on the FMAs).
+# Per (tetrahedron, band): 40 + 5*norb as above + H, J of the two outer intervals, 2 * 11*norb.
+def flops_alg_gen5(n_eval: int, n_mid: int, n_tb: int, norb: int) -> float:
+    return (float(n_eval - n_mid) * (8 * norb + 8) + float(n_mid) * (70 + 16 * norb)
+            + float(n_tb) * (40 + 5 * norb + 22 * norb))
 
 
 # FP32-ALU peak derived from the guide's unit counts and clocks: SMs x 128 FP32 lanes x 2 flops (FMA)
@@ -175,7 +186,8 @@ def workload_config(cfg, n_gpus: int) -> dict:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the main kernel, from the committed
 # `ncu --set full` capture (profiles/, named there); None until a capture of that config exists.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {("cfg4", 3): 1.394956e9 + 280.968e6,    # profiles/r01_v3_regions_cfg4.md
+                     ("cfg4", 5): 1.099610e9 + 209.691e6}    # profiles/r01_v5_main_cfg4.md
 
 
 def main():
@@ -252,13 +264,14 @@ def main():
     # ---- work counters (exact integers from the kernel) and per-kernel device times of the timed steps
     main_ms, merge_ms = plan.kernel_ms(min(args.steps, 64))
     cnt = plan.last_counters()
-    c = torch.tensor([cnt["n_tb"], cnt["n_eval"]], dtype=torch.int64, device=dev)
+    gen = int(cnt["kernel"])
+    c = torch.tensor([cnt["n_tb"], cnt["n_eval"], max(cnt["n_eval_mid"], 0)], dtype=torch.int64, device=dev)
     if world > 1:
         dist.all_reduce(c)
         km = torch.tensor([main_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(km, op=dist.ReduceOp.MAX)
         main_ms = float(km.item())
-    n_tb, n_eval = int(c[0].item()), int(c[1].item())
+    n_tb, n_eval, n_mid = int(c[0].item()), int(c[1].item()), int(c[2].item())
     info = plan.info()
     launches_per_step = 3   # main + merge + finalize (memsets and NCCL not counted)
 
@@ -315,11 +328,15 @@ def main():
     props = torch.cuda.get_device_properties(dev)
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak = fp32_peak_tflops(props.multi_processor_count, sm_max)
-    fl = flops_alg(n_eval, n_tb, norb) / world          # per launch (each rank's share on average)
+    fl_paper = flops_alg(n_eval, n_tb, norb) / world    # per launch (each rank's share on average)
+    fl = flops_alg_gen5(n_eval, n_mid, n_tb, norb) / world if gen == 5 else fl_paper
     achieved = fl / (main_ms * 1e-3) / 1e12
     bytes_alg = 4.0 * N1 * N2 * N3 * nb * (1 + (0 if unitW else norb)) + 8.0 * norb * nE
-    roofline = {"bound": "alu", "kernel": "tdos_main", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+    roofline = {"bound": "alu", "kernel": "tdos_main5" if gen == 5 else "tdos_main", "achieved": achieved, "peak": peak,
+                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, gen)),
+                "flop_model": "generation-5 formulation (H, J hoisted for Eq. 12/14)" if gen == 5 else "paper formulation",
+                "frac_paper_formulation": fl_paper / (main_ms * 1e-3) / 1e12 / peak,
+                "flops_paper_formulation_per_launch": fl_paper,
                 "peak_source": "derived: %d SMs x 128 FP32 lanes x 2 x %.0f MHz (B200_PROFILING.md unit counts and clocks)"
                                % (props.multi_processor_count, sm_max),
                 "flops_alg_per_launch": fl, "main_kernel_ms": main_ms, "merge_finalize_ms": merge_ms,
@@ -337,7 +354,7 @@ def main():
                        if bytes_alg > 126e6 else "inputs fit in L2; L2 not flushed between steps",
                        tile=list(info["tile"]), grid=info["grid"], threads=info["threads"], smem=info["smem"]),
         "effective_evals_per_s": n_eval / (ms_per_step * 1e-3), "dos_grids_per_s": 1e3 / ms_per_step,
-        "n_tb": n_tb, "n_eval": n_eval,
+        "n_tb": n_tb, "n_eval": n_eval, "n_eval_mid": n_mid if gen >= 4 else None, "kernel_generation": gen,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
     }
 

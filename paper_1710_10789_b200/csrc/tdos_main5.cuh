@@ -75,7 +75,13 @@ struct AccE {
             red_add4(row + (size_t)b * 3 * norb, D[b][0].x, D[b][0].y, D[b][1].x, D[b][1].y);
             red_add4(row + (size_t)b * 3 * norb + norb, T[b][0].x, T[b][0].y, T[b][1].x, T[b][1].y);
         }
-        zero();
+        clear();
+    }
+    // back to zero after a flush: one packed multiply per register pair (the sums are finite)
+    __device__ __forceinline__ void clear() {
+        const f2 Z = dup(0.0f);
+#pragma unroll
+        for (int b = 0; b < 4; b++) { D[b][0] = mul2(D[b][0], Z); D[b][1] = mul2(D[b][1], Z); T[b][0] = mul2(T[b][0], Z); T[b][1] = mul2(T[b][1], Z); }
     }
 };
 
@@ -118,7 +124,11 @@ struct AccM {
                 red_add4(r + norb + 4, T[b][2].x, T[b][2].y, T[b][3].x, T[b][3].y);
             }
         }
-        zero();
+        const f2 Z = dup(0.0f);
+#pragma unroll
+        for (int b = 0; b < 2; b++)
+#pragma unroll
+            for (int j = 0; j < 4; j++) { D[b][j] = mul2(D[b][j], Z); T[b][j] = mul2(T[b][j], Z); }
     }
 };
 
@@ -307,7 +317,7 @@ __device__ __forceinline__ void walk5(unsigned char* __restrict__ base, float* _
             if (m == 0) {
                 if (wm == 0) {   // the group leaves chunk c
                     float* row = prow + (size_t)(c * CH + lb) * 3 * norb;
-                    if constexpr (KIND == 0) { if (live) accE.flush(row, norb); else accE.zero(); }
+                    if constexpr (KIND == 0) { if (live) accE.flush(row, norb); else accE.clear(); }
                     else accM.flush(row, norb, second);
                     do {
                         ++c;
