@@ -44,6 +44,7 @@ struct MainParams {
     int nmb;                     // orbital blocks of MB
     int n_items;                 // ntx*nty*ntz*nb*nmb
     int unitW;                   // W == 1
+    int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
     float* partial;              // [gridDim.x] x { D[norb][nE], T[norb][nE], S[nE][norb] }
     unsigned long long* counters;   // [0] n_tb, [1] n_eval = #(tb, omega) with E1 < omega < E4
 };

@@ -25,6 +25,22 @@
 
 namespace tdos {
 
+// locate_bin (tdos_kernels.cuh) on an energy array in any address space (shared-memory copy or global)
+template <bool STRICT>
+__device__ __forceinline__ int locate5(const float* om, int nE, float om0, float inv_dom, float x) {
+    float gq = (x - om0) * inv_dom;
+    gq = fminf(fmaxf(gq, 0.0f), (float)nE);
+    int i = (int)gq;
+    if (STRICT) {
+        while (i > 0 && om[i - 1] > x) --i;
+        while (i < nE && om[i] <= x) ++i;
+    } else {
+        while (i > 0 && om[i - 1] >= x) --i;
+        while (i < nE && om[i] < x) ++i;
+    }
+    return i;
+}
+
 template <int TX, int TY, int TZ>
 struct Cfg5 {
     static constexpr int MB = 8;
@@ -401,6 +417,14 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
 
     const int nE = p.nE, norb = NORB ? NORB : p.norb;
     const float* __restrict__ omega = p.omega;
+    // the energy grid is probed 8 times per (tetrahedron, band): keep a block-wide copy in shared memory when it fits
+    const float* om_loc = omega;
+    if (p.om_smem) {
+        float* sOmAll = reinterpret_cast<float*>(smem + (size_t)NWARP * C::bytes);
+        for (int i = threadIdx.x; i < nE; i += NWARP * 32) sOmAll[i] = __ldg(omega + i);
+        __syncthreads();
+        om_loc = sOmAll;
+    }
     const float om0 = __ldg(omega);
     float inv_dom = 0.0f;
     if (nE > 1) {
@@ -487,10 +511,10 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
                 uint32_t rl = 0, rh = 0, rm = 0;               // empty ranges
                 if (valid) {
                     // bins (reading G10): low [i1,i2), mid [i2,i3), high [i3,i4), full weight from i4 on
-                    const int i1 = locate_bin<true>(omega, nE, om0, inv_dom, e0);             // first omega > E1
-                    const int i2 = max(i1, locate_bin<false>(omega, nE, om0, inv_dom, e1));   // first omega >= E2
-                    const int i3 = max(i2, locate_bin<false>(omega, nE, om0, inv_dom, e2));
-                    const int i4 = max(i3, locate_bin<false>(omega, nE, om0, inv_dom, e3));
+                    const int i1 = locate5<true>(om_loc, nE, om0, inv_dom, e0);             // first omega > E1
+                    const int i2 = max(i1, locate5<false>(om_loc, nE, om0, inv_dom, e1));   // first omega >= E2
+                    const int i3 = max(i2, locate5<false>(om_loc, nE, om0, inv_dom, e2));
+                    const int i4 = max(i3, locate5<false>(om_loc, nE, om0, inv_dom, e3));
                     rl = (uint32_t)i1 | ((uint32_t)i2 << 16);
                     rm = (uint32_t)i2 | ((uint32_t)i3 << 16);
                     rh = (uint32_t)i3 | ((uint32_t)i4 << 16);

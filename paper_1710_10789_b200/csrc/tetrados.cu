@@ -110,6 +110,7 @@ struct tdos_plan {
     int nk[3] = {0, 0, 0};
     int nb = 0, norb = 0, nE_max = 0;
     int num_sms = 0;
+    size_t smem_optin = 0;        // cudaDevAttrMaxSharedMemoryPerBlockOptin
     Variant var{};
     int blocks_per_sm = 0;
     int grid = 0;
@@ -198,6 +199,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     p->norb = norb;
     p->nE_max = nE_max;
     p->num_sms = prop.multiProcessorCount;
+    p->smem_optin = prop.sharedMemPerBlockOptin;
 
     const char* kv = getenv("TDOS_KERNEL");
     // generation 5 needs blocks of 8 orbitals to pay off; narrower problems use generation 3
@@ -210,7 +212,10 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     p->var = vs[sel];
 
     const void* kfn = p->var.fn4 ? (const void*)p->var.fn4 : (const void*)p->var.fn;
-    cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->var.smem);
+    size_t smem_attr = p->var.smem;
+    if (p->var.gen == 5 && p->var.smem + (size_t)nE_max * sizeof(float) <= p->smem_optin)
+        smem_attr += (size_t)nE_max * sizeof(float);
+    cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_attr);
     if (e == cudaSuccess)
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->blocks_per_sm, kfn, p->var.NWARP * 32, p->var.smem);
     if (e != cudaSuccess || p->blocks_per_sm < 1) {
@@ -306,6 +311,12 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         m4.n_batches = (int)work;
         m4.next_batch = reinterpret_cast<unsigned int*>(p->counters + 3);
     }
+    // generation 5: a block-wide copy of omega in shared memory if the device limit allows it
+    size_t smem = v.smem;
+    if (v.gen == 5 && v.smem + (size_t)nE * sizeof(float) <= p->smem_optin) {
+        mp.om_smem = 1;
+        smem += (size_t)nE * sizeof(float);
+    }
     const size_t hist = (size_t)3 * p->norb * mp.nEp;
     if (first) {
         CK(cudaMemsetAsync(p->partial, 0, hist * p->grid * sizeof(float), st));
@@ -322,7 +333,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
             m4.b = mp;
             v.fn4<<<grid, v.NWARP * 32, v.smem, st>>>(m4);
         } else {
-            v.fn<<<grid, v.NWARP * 32, v.smem, st>>>(mp);
+            v.fn<<<grid, v.NWARP * 32, smem, st>>>(mp);
         }
         CK(cudaGetLastError());
         p->last_launches += 1;
