@@ -46,6 +46,7 @@ struct MainParams {
     int unitW;                   // W == 1
     int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
     float* partial;              // [gridDim.x] x { D[norb][nE], T[norb][nE], S[nE][norb] }
+    unsigned int* next_item;        // tdos_main5: work counter, zero at launch
     unsigned long long* counters;   // [0] n_tb, [1] n_eval = #(tb, omega) with E1 < omega < E4
 };
 

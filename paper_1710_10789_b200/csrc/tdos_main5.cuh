@@ -437,8 +437,12 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
     float* sOm = reinterpret_cast<float*>(base + C::off_om);
     unsigned long long cnt_tb = 0, cnt_ev = 0, cnt_mid = 0;
 
-    const int gwarp = blockIdx.x * NWARP + warp, nwarps = gridDim.x * NWARP;
-    for (int item = gwarp; item < p.n_items; item += nwarps) {
+    // warps draw items from a global counter (windows differ from band to band: a static split leaves SMs idle at the end)
+    for (;;) {
+        int item = 0;
+        if (lane == 0) item = (int)atomicAdd(p.next_item, 1u);
+        item = __shfl_sync(FULL, item, 0);
+        if (item >= p.n_items) break;
         // ---- decode the work item (orbital block, band fastest: neighbouring warps share the tile's lines)
         int r = item;
         const int mb = r % p.nmb; r /= p.nmb;

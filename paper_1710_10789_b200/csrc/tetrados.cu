@@ -302,6 +302,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     mp.unitW = (W == nullptr);
     mp.partial = p->partial;
     mp.counters = p->counters;
+    mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
 
     Main4Params m4{};
     long long work = items;   // independent units the warps draw: items (v3) or batches of tiles (v4)
@@ -323,7 +324,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         CK(cudaMemsetAsync(p->counters, 0, 4 * sizeof(unsigned long long), st));
         p->last_items = 0;
         p->last_launches = 0;
-    } else if (v.fn4) {
+    } else if (v.gen >= 4) {
         CK(cudaMemsetAsync(p->counters + 3, 0, sizeof(unsigned long long), st));
     }
     if (work > 0) {
