@@ -136,13 +136,17 @@ def oracle_sample_planes(cfg) -> int:
     return max(1, cfg.nk[2] // 16)
 
 
-def run_oracle_sample(cfg, E, W, om, reps: int = 1, warmup: int = 0):
-    """Time the fp64 oracle, as it stands, on the sample.  Returns (seconds per rep, n_tb, n_eval, cores, text)."""
+def run_oracle_sample(cfg, E, W, om, reps: int = 1, warmup: int = 0, single_core: bool = False):
+    """Time the fp64 oracle, as it stands, on the sample.  Returns (seconds per rep, n_tb, n_eval, cores, text).
+    single_core: one thread on 1/8 of the sample's planes (comparable in spirit with the paper's single-core
+    CPU reference)."""
     import oracle
     oracle.build()
     planes = oracle_sample_planes(cfg)
+    if single_core:
+        planes = max(1, planes // 8)
     hi = cfg.nk[0] * cfg.nk[1] * planes
-    cores = min(oracle.max_threads(), len(os.sched_getaffinity(0)))
+    cores = 1 if single_core else min(oracle.max_threads(), len(os.sched_getaffinity(0)))
     Wn = None if cfg.model == "cosine" else W
     times, res = [], None
     for r in range(warmup + reps):
@@ -362,6 +366,9 @@ def main():
         sec, s_tb, s_eval, cores, text = run_oracle_sample(cfg, E, W, om)
         line["cpu_baseline"] = {"value": s_tb * nE / sec, "unit": "eval/s", "cores": cores, "kind": "oracle",
                                 "sample": text, "seconds": sec, "effective_evals_per_s": s_eval / sec}
+        sec1, t_tb, t_eval, _, text1 = run_oracle_sample(cfg, E, W, om, single_core=True)
+        line["cpu_baseline"]["single_core"] = {"value": t_tb * nE / sec1, "unit": "eval/s", "cores": 1, "sample": text1,
+                                               "seconds": sec1, "effective_evals_per_s": t_eval / sec1}
     if rank == 0:
         print(json.dumps(line), flush=True)
     plan.close()

@@ -252,3 +252,36 @@ def test_experimental_kernel_generation_4(monkeypatch):
 def test_paper_shaped_anisotropic_grid(cache_dir):
     """60 x 60 x 10 k-points, 8 bands, 1024 energies (the shapes of Table II's last row)."""
     _full_config("paper60", cache_dir)
+
+
+@pytest.mark.parametrize("nk,nb,norb,nE", [
+    ((4, 4, 8), 2, 8, 1),         # a single energy
+    ((3, 5, 2), 1, 8, 3),         # fewer energies than a chunk of 4 bins, ragged against every tile
+    ((6, 4, 16), 2, 8, 130),      # windows cross the 128-bin pass boundary
+    ((2, 2, 2), 3, 16, 61),       # two orbital blocks, every neighbour is a wrap
+    ((7, 6, 9), 2, 12, 515),      # second orbital block half empty (norb = 12)
+])
+def test_generation5_edge_cases(nk, nb, norb, nE):
+    """The default kernel for norb % 4 == 0, norb >= 5 (tdos_main5) on the degenerate shapes: AoS, SoA, host mode,
+    random energies (windows of many bins) and lattice energies with omega ON the corner values (ties, G10/G11)."""
+    E, W = wl.random_bands(nk, nb, norb, seed=7 + nE)
+    om = wl.omega_grid(-1.1, 1.2, nE)
+    ref = oracle.tetra_dos(E, W, nk, om)
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        dos, nos = run_gpu(E, W, nk, om, plan=plan)
+        cnt = plan.last_counters()
+    assert cnt["kernel"] == 5 and cnt["n_tb"] == ref["n_tb"] and cnt["n_eval"] == ref["n_eval"]
+    assert cnt["n_eval_mid"] == ref["n_case"][1]
+    assert_parity(ref, dos, nos, "gen5 %s" % (nk,))
+    Es, Ws = wl.to_soa(E, W)
+    dos, nos = run_gpu(Es, Ws, nk, om, layout=binding.TDOS_SOA)
+    assert_parity(ref, dos, nos, "gen5 SoA %s" % (nk,))
+    dos, nos = run_gpu(E, W, nk, om, memspace=binding.TDOS_HOST)
+    assert_parity(ref, dos, nos, "gen5 host %s" % (nk,))
+    rng = np.random.default_rng(nE)
+    n = int(np.prod(nk))
+    E2 = np.sort(rng.integers(-8, 9, (n, nb)) / 8.0, axis=1).astype(np.float32)
+    om2 = np.unique(np.concatenate([om, (np.arange(-9, 10) / 8.0).astype(np.float32)]))[:max(nE, 1)]
+    ref2 = oracle.tetra_dos(E2, W, nk, om2)
+    dos, nos = run_gpu(E2, W, nk, om2)
+    assert_parity(ref2, dos, nos, "gen5 ties %s" % (nk,))
