@@ -102,7 +102,7 @@ int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const fl
 /*
  * Multi-GPU building blocks (device pointers only).
  * tetra_dos_partial: the additive share of the cubes with z_lo <= iz < z_hi, as raw fp64 sums
- *   part[3][norb][nE]  (0: sum b*dw/V, 1: in-window sum b*w/V, 2: Eq.-15 step histogram / V),
+ *   part[3][norb][nE]  (0: sum b*dw/V, 1: sum b*w/V over E1 < omega < E4, 2: Eq.-15 step histogram / V at the first omega >= E4),
  *   overwritten.  E and W must hold the whole grid (the kernel reads planes z_lo .. z_hi, wrapping).
  * tetra_dos_finalize: dos = V*part[0]; nos = V*(part[1] + inclusive prefix sum over omega of part[2]).
  * A sum of the `part` arrays of disjoint slabs covering 0..N3 (e.g. an all-reduce) followed by

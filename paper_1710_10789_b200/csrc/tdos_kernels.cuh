@@ -335,8 +335,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 c0 *= WST; c1 *= WST; c2 *= WST; c3 *= WST;   // float offsets into sW
                 if (valid) {
                     const int i1 = locate_bin<true>(omega, nE, om0, inv_dom, e0);      // first omega > E1
-                    // first omega >= E3 / >= E4, and > E1 (test order G10)
-                    const int i3 = (e2 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e2) : i1;
+                    // first omega >= E4, and > E1 (test order G10)
                     const int i4 = (e3 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e3) : i1;
                     rng = (uint32_t)i1 | ((uint32_t)i4 << 16);
                     if (mb == 0) {   // work counters (exact integers; bench.py's flop count uses them)
@@ -347,16 +346,16 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                         lmin = min(lmin, i1);
                         lmax = max(lmax, i4 - 1);
                     }
-                    // Eq. 14c/e and Eq. 15 (A6): from the first omega >= E3 on, every corner carries the constant
-                    // V (Eq. 14 adds -C y/E_4j to it inside the window): one add of sum_l b_l into the
-                    // step histogram at bin i3
-                    if (i3 < nE) {
+                    // Eq. 15 (A6): from the first omega >= E4 on, every corner carries the constant
+                    // V: one add of sum_l b_l into the
+                    // step histogram at bin i4 (all fp32 sums stay sums of non-negative terms)
+                    if (i4 < nE) {
                         float b0[MB], b1[MB], b2[MB], b3[MB];
                         load_b<MB>(sW + c0, b0);
                         load_b<MB>(sW + c1, b1);
                         load_b<MB>(sW + c2, b2);
                         load_b<MB>(sW + c3, b3);
-                        float* dst = part + (size_t)i3 * 3 * norb + 2 * norb + m0;
+                        float* dst = part + (size_t)i4 * 3 * norb + 2 * norb + m0;
                         if (vec4) {
                             if constexpr (MB % 4 == 0) {
 #pragma unroll

@@ -9,14 +9,17 @@
 //     [i1,i2), mid [i2,i3), high [i3,i4) in bins.  Low and high records are walked in one phase, mid records
 //     in a second one, so all lanes of a warp run the same code;
 //   * low / high (Eq. 12 and its mirror image Eq. 14): with s = (w-e1)/e21 (or (e4-w)/e43) Eq. 8 (:91) becomes
-//         T_m = sum_l b_lm w_l = s^3 H_m + s^4 J_m,   H_m = 4 rho b_near,m,  J_m = rho sum_far q_j (b_j,m - b_near,m)
+//         T_m = sum_l b_lm w_l = s^3 H_m + s^4 J_m   (low),      T_m = sum_l b_lm - (s^3 H_m + s^4 J_m)   (high),
+//         H_m = 4 rho b_near,m,  J_m = rho sum_far q_j (b_j,m - b_near,m)
 //     with q_j = e21/e_j1, rho = q_3 q_4 (all ratios <= 1), and D_m = dT_m/dw from the same H, J.  H and J are
 //     formed once per (record, chunk) step from the four corners' orbital weights, then every bin costs
 //     4 FMAs per orbital instead of 8 plus the weights.  A group of 2 lanes owns 4 bins, lane h the
 //     orbitals 4h..4h+3;
 //   * mid (Eq. 13a-n): the weights w_l, dw_l are evaluated as in v3 (tdos_weights.cuh's middle path, alone),
 //     followed by the 4 x 8 projection; lanes own 2 bins x 8 orbitals.
-// Eq. 14's constant sum_l b_l and Eq. 15 go into the step histogram S at the first energy >= e3, as before.
+// Only Eq. 15 (a finished tetrahedron: sum_l b_l for every energy >= e4) goes into the step histogram S; inside
+// [e3, e4) the constant of Eq. 14c/e is accumulated with the rest, so that every fp32 sum (registers, block
+// partials, S) is a sum of non-negative terms and none of them can exceed N itself.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -149,12 +152,15 @@ struct AccM {
 };
 
 // One low/high step.  bN, b1, b2, b3: orbital weights (this lane's 4 orbitals) at the near corner and at the far
-// corners with ratios 1, qa, qb;  x0 = e1 (low) / e4 (high);  r = 1/e21 / -1/e43;  rs = rho (low) / -rho (high).
+// corners with ratios 1, qa, qb;  x0 = e1 (low) / e4 (high);  r = 1/e21 / -1/e43;  rs = rho (low) / -rho (high);
+// hi1 = 0 (low) / 1 (high): Eq. 14c/e's constant sum_l b_l.
 __device__ __forceinline__ void eval_edge5(AccE& a, const float4 bN, const float4 b1, const float4 b2, const float4 b3,
-                                           float qa, float qb, float rs, float x0, float r, const f2 (&om)[2],
+                                           float qa, float qb, float rs, float x0, float r, float hi1, const f2 (&om)[2],
                                            const bool (&ok)[4]) {
     const f2 N01 = make_float2(bN.x, bN.y), N23 = make_float2(bN.z, bN.w);
     const f2 NEG = dup(-1.0f);
+    const f2 V01 = add2(add2(N01, make_float2(b1.x, b1.y)), add2(make_float2(b2.x, b2.y), make_float2(b3.x, b3.y)));
+    const f2 V23 = add2(add2(N23, make_float2(b1.z, b1.w)), add2(make_float2(b2.z, b2.w), make_float2(b3.z, b3.w)));
     // G = (b1 - bN) + qa (b2 - bN) + qb (b3 - bN)
     f2 G01 = fma2(N01, NEG, make_float2(b1.x, b1.y)), G23 = fma2(N23, NEG, make_float2(b1.z, b1.w));
     G01 = fma2(fma2(N01, NEG, make_float2(b2.x, b2.y)), dup(qa), G01);
@@ -175,6 +181,8 @@ __device__ __forceinline__ void eval_edge5(AccE& a, const float4 bN, const float
         for (int e = 0; e < 2; e++) {
             const int b = 2 * pr + e;
             const float t3 = e ? s3.y : s3.x, t4 = e ? s4.y : s4.x, g2 = e ? d2.y : d2.x, g3 = e ? d3.y : d3.x;
+            const float one = ok[b] ? hi1 : 0.0f;
+            a.T[b][0] = fma2(V01, dup(one), a.T[b][0]); a.T[b][1] = fma2(V23, dup(one), a.T[b][1]);
             a.T[b][0] = fma2(H01, dup(t3), a.T[b][0]); a.T[b][1] = fma2(H23, dup(t3), a.T[b][1]);
             a.T[b][0] = fma2(J01, dup(t4), a.T[b][0]); a.T[b][1] = fma2(J23, dup(t4), a.T[b][1]);
             a.D[b][0] = fma2(H01, dup(g2), a.D[b][0]); a.D[b][1] = fma2(H23, dup(g2), a.D[b][1]);
@@ -379,7 +387,7 @@ __device__ __forceinline__ void walk5(unsigned char* __restrict__ base, float* _
                 const float4 b1 = *reinterpret_cast<const float4*>(wb + (u >> 16));
                 const float4 b2 = *reinterpret_cast<const float4*>(wb + (v & 0xffffu));
                 const float4 b3 = *reinterpret_cast<const float4*>(wb + (v >> 16));
-                eval_edge5(accE, bN, b1, b2, b3, qa, qb, hiK ? -rho : rho, hiK ? es.w : es.x, hiK ? -r0 : r0, om, ok);
+                eval_edge5(accE, bN, b1, b2, b3, qa, qb, hiK ? -rho : rho, hiK ? es.w : es.x, hiK ? -r0 : r0, hiK ? 1.0f : 0.0f, om, ok);
             } else {
                 const float4 es = sEs[t];
                 const uint2 cs = sCs[t];
@@ -403,7 +411,7 @@ __device__ __forceinline__ void walk5(unsigned char* __restrict__ base, float* _
 template <int TX, int TY, int TZ, int NWARP, int NORB>
 __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) {
     using C = Cfg5<TX, TY, TZ>;
-    constexpr int PX = C::PX, PY = C::PY, PK = C::PK, NC = C::NC, NTB = C::NTB, WST = C::WST, MB = C::MB;
+    constexpr int PX = C::PX, PY = C::PY, PK = C::PK, NTB = C::NTB, WST = C::WST, MB = C::MB;
     constexpr unsigned FULL = 0xffffffffu;
 
     extern __shared__ __align__(16) unsigned char smem[];
@@ -531,15 +539,15 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
                         lmin = min(lmin, i1);
                         lmax = max(lmax, i4 - 1);
                     }
-                    // Eq. 14c/e and Eq. 15 (A6): from the first omega >= E3 on every corner carries the constant V:
-                    // one add of sum_l b_l into the step histogram at bin i3 (prefix-summed in fp64 later)
-                    if (i3 < nE) {
+                    // Eq. 15 (A6): from the first omega >= E4 on every corner carries the constant V:
+                    // one add of sum_l b_l into the step histogram at bin i4 (prefix-summed in fp64 later)
+                    if (i4 < nE) {
                         float b0[8], b1[8], b2[8], b3[8];
                         load_b<8>(sW + c0, b0);
                         load_b<8>(sW + c1, b1);
                         load_b<8>(sW + c2, b2);
                         load_b<8>(sW + c3, b3);
-                        float* dst = part + (size_t)i3 * 3 * norb + 2 * norb + m0;
+                        float* dst = part + (size_t)i4 * 3 * norb + 2 * norb + m0;
 #pragma unroll
                         for (int m4 = 0; m4 < 8; m4 += 4)
                             if (m0 + m4 < norb)

@@ -7,8 +7,8 @@
 //     the finalize kernel);
 //   * Eq. 12 and Eq. 14 are mirror images (E - E1 <-> E4 - E, corners 1,2,3,4 <-> 4,3,2,1): one code path
 //     ("edge") serves both, its inputs selected per energy;
-//   * Eq. 14's weights are returned as w_j - V (= -C q_j): the constant V of Eq. 14c/e is added by the
-//     caller as a step at the first energy >= E3, together with Eq. 15's;
+//   * Eq. 14's weights are formed as w_j = V - C q_j (Eq. 14c/e as printed); only Eq. 15's constant (a finished
+//     tetrahedron) is added by the caller as a step at the first energy >= E4;
 //   * the derivative identities  sum_l dw_l = 4 dC  (Eq. 12) / -4 dC (Eq. 14)  replace 12d and 14f;
 //   * misprints of the paper are read as in DESIGN.md (G1-G5).
 // The two energies of a call may fall in different intervals: the edge path and the middle path (Eq. 13)
@@ -33,7 +33,7 @@ __device__ __forceinline__ float rcp_fast(float x) {
 }
 
 // Sorted corner energies e1 <= e2 <= e3 <= e4 and two energies E = (Ea, Eb).
-// For each energy with e1 < E < e4:  w[l] = w_l/V (E < e3) or w_l/V - 1 (E >= e3),  dw[l] = (dw_l/dE)/V,
+// For each energy with e1 < E < e4:  w[l] = w_l/V,  dw[l] = (dw_l/dE)/V,
 // for the sorted corners l = 0..3; for an energy outside (e1, e4), or NaN, all eight values are 0.
 __device__ __forceinline__ void corner_weights_x2(float e1, float e2, float e3, float e4, f2 E, f2 (&w)[4], f2 (&dw)[4]) {
     const bool va = (E.x > e1) && (E.x < e4), vb = (E.y > e1) && (E.y < e4);
@@ -80,6 +80,10 @@ __device__ __forceinline__ void corner_weights_x2(float e1, float e2, float e3, 
         w[3].x = lo_a ? wF3.x : wN.x;   w[3].y = lo_b ? wF3.y : wN.y;
         dw[0].x = lo_a ? dN.x : dF3.x;  dw[0].y = lo_b ? dN.y : dF3.y;
         dw[3].x = lo_a ? dF3.x : dN.x;  dw[3].y = lo_b ? dF3.y : dN.y;
+        // Eq. 14c/e: w_j = V - C q_j for an energy in [E3, E4)
+        const f2 ONE = make_float2((ed_a && !lo_a) ? 1.0f : 0.0f, (ed_b && !lo_b) ? 1.0f : 0.0f);
+#pragma unroll
+        for (int l = 0; l < 4; l++) w[l] = add2(w[l], ONE);
     }
     if (mi_a || mi_b) {
         // ---- Eq. 13.  For an energy this path does not serve, a = b = 0 makes every term vanish.

@@ -13,7 +13,6 @@
 #include <vector>
 
 #include "tdos_kernels.cuh"
-#include "tdos_main4.cuh"
 #include "tdos_main5.cuh"
 
 namespace {
@@ -34,18 +33,14 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
-using tdos::Main4Params;
 using tdos::MainParams;
 typedef void (*main_kernel_t)(const MainParams);
-typedef void (*main4_kernel_t)(const Main4Params);
 
 struct Variant {
-    main_kernel_t fn;      // v3 kernel (default), or null
+    main_kernel_t fn;      // tdos_main (generation 3) or tdos_main5 (generation 5)
     int MB, TX, TY, TZ, GL, NWARP;
     size_t smem;
-    main4_kernel_t fn4 = nullptr;   // v4 kernel (TDOS_KERNEL=4, experimental: DESIGN.md 4.2)
-    int BX = 0;                     // v4: tiles per batch
-    int gen = 3;                    // main kernel generation: 3, 4 or 5
+    int gen = 3;                    // main kernel generation: 3 or 5
 };
 
 template <int TX, int TY, int TZ, int NWARP, int NORB>
@@ -62,20 +57,6 @@ template <int NORB>
 std::vector<Variant> variants5() {
     return {make_variant5<4, 4, 2, 16, NORB>(), make_variant5<2, 2, 8, 16, NORB>(), make_variant5<4, 2, 4, 16, NORB>(),
             make_variant5<4, 4, 2, 12, NORB>(), make_variant5<4, 4, 1, 16, NORB>()};
-}
-
-template <int TX, int TY, int TZ, int NWARP>
-Variant make_variant4() {
-    Variant v{nullptr, 8, TX, TY, TZ, 2, NWARP, (size_t)NWARP * tdos::Cfg4<TX, TY, TZ>::bytes};
-    v.fn4 = tdos::tdos_main4<TX, TY, TZ, NWARP>;
-    v.BX = tdos::Cfg4<TX, TY, TZ>::BX;
-    v.gen = 4;
-    return v;
-}
-
-// v4 configurations compiled in (TDOS_TILE=<index> selects another one for experiments)
-std::vector<Variant> variants4() {
-    return {make_variant4<2, 2, 2, 8>(), make_variant4<4, 2, 1, 8>(), make_variant4<2, 2, 1, 12>()};
 }
 
 template <int MB, int TX, int TY, int TZ, int GL, int NWARP>
@@ -206,7 +187,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     // generation 5 needs blocks of 8 orbitals to pay off; narrower problems use generation 3
     int gen = kv ? atoi(kv) : 5;
     if (gen == 5 && (norb < 5 || norb % 4 != 0)) gen = 3;   // tdos_main5: blocks of 8 orbitals, 16-byte vector reductions
-    std::vector<Variant> vs = gen == 4 ? variants4() : gen == 5 ? (norb == 8 ? variants5<8>() : variants5<0>()) : variants(pick_mb(norb));
+    std::vector<Variant> vs = gen == 5 ? (norb == 8 ? variants5<8>() : variants5<0>()) : variants(pick_mb(norb));
     int sel = 0;
     // Tile shape of generation 5.  A tile whose bands span few energy bins keeps more (record, chunk) entries per
     // chunk.  The paper's workloads are layered materials sampled on grids like 60 x 60 x 10, with
@@ -217,7 +198,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     if (sel < 0 || sel >= (int)vs.size()) sel = 0;
     p->var = vs[sel];
 
-    const void* kfn = p->var.fn4 ? (const void*)p->var.fn4 : (const void*)p->var.fn;
+    const void* kfn = (const void*)p->var.fn;
     size_t smem_attr = p->var.smem;
     if (p->var.gen == 5 && p->var.smem + (size_t)nE_max * sizeof(float) <= p->smem_optin)
         smem_attr += (size_t)nE_max * sizeof(float);
@@ -310,14 +291,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     mp.counters = p->counters;
     mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
 
-    Main4Params m4{};
-    long long work = items;   // independent units the warps draw: items (v3) or batches of tiles (v4)
-    if (v.fn4) {
-        m4.nbx = (mp.ntx + v.BX - 1) / v.BX;
-        work = (long long)m4.nbx * mp.nty * mp.ntz * p->nb * mp.nmb;
-        m4.n_batches = (int)work;
-        m4.next_batch = reinterpret_cast<unsigned int*>(p->counters + 3);
-    }
+    const long long work = items;
     // generation 5: a block-wide copy of omega in shared memory if the device limit allows it
     size_t smem = v.smem;
     if (v.gen == 5 && v.smem + (size_t)nE * sizeof(float) <= p->smem_optin) {
@@ -330,18 +304,13 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         CK(cudaMemsetAsync(p->counters, 0, 4 * sizeof(unsigned long long), st));
         p->last_items = 0;
         p->last_launches = 0;
-    } else if (v.gen >= 4) {
+    } else if (v.gen == 5) {
         CK(cudaMemsetAsync(p->counters + 3, 0, sizeof(unsigned long long), st));
     }
     if (work > 0) {
         const long long blocks_needed = (work + v.NWARP - 1) / v.NWARP;
         const int grid = (int)((blocks_needed < p->grid) ? blocks_needed : p->grid);
-        if (v.fn4) {
-            m4.b = mp;
-            v.fn4<<<grid, v.NWARP * 32, v.smem, st>>>(m4);
-        } else {
-            v.fn<<<grid, v.NWARP * 32, smem, st>>>(mp);
-        }
+        v.fn<<<grid, v.NWARP * 32, smem, st>>>(mp);
         CK(cudaGetLastError());
         p->last_launches += 1;
     }
@@ -539,7 +508,7 @@ int tdos_last_counters(tdos_plan* p, long long cnt[4]) {
     CK(cudaMemcpy(h, p->counters, sizeof(h), cudaMemcpyDeviceToHost));
     cnt[0] = (long long)h[0];
     cnt[1] = (long long)h[1];
-    cnt[2] = p->var.gen >= 4 ? (long long)h[2] : -1;
+    cnt[2] = p->var.gen == 5 ? (long long)h[2] : -1;
     cnt[3] = p->var.gen;
     return TDOS_OK;
 }
