@@ -191,7 +191,7 @@ def workload_config(cfg, n_gpus: int) -> dict:
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the main kernel, from the committed
 # `ncu --set full` capture (profiles/, named there); None until a capture of that config exists.
 NCU_TRAFFIC_BYTES = {("cfg4", 3): 1.394956e9 + 280.968e6,    # profiles/r01_v3_regions_cfg4.md
-                     ("cfg4", 5): 1.089019e9 + 206.889e6}    # profiles/r01_v5_main_cfg4.md
+                     ("cfg4", 5): 731.369e6 + 80.145e6}    # profiles/r01_v5_main_cfg4.md
 
 
 def main():
