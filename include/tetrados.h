@@ -25,6 +25,10 @@
  *                   partial sums, fp64 merge across blocks and fp64 prefix sum for N; fp32 outputs.
  *   NaN/Inf in E or W are not detected: results are then undefined.
  *
+ * Kernels: tdos_main5 (one record per interval of Eq. 12-14; norb >= 5 and norb % 4 == 0) or tdos_main (any norb);
+ * the environment variables TDOS_KERNEL=3|5 and TDOS_TILE=<index>, read at plan creation, override the choice of
+ * kernel and tile shape for experiments.
+ *
  * Ownership: the caller owns every array; the library never frees them and does not retain them
  * past the call (device mode: past completion of the work queued on `stream`).  A plan owns all
  * scratch (block partials, staging buffers, its side stream).  A plan must not be used from two
