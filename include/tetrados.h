@@ -104,6 +104,15 @@ int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const fl
               float* dos, float* nos, int memspace, void* cuda_stream);
 
 /*
+ * The same with the eigenvector elements themselves (Eq. 1-3, :37-48; the paper's kernel takes real and
+ * imaginary parts, :263): A holds nk*nb*norb complex numbers as (re, im) float pairs in `layout`
+ * (TDOS_AOS: A[ik][n][m][2], TDOS_SOA: A[n][m][ik][2]); the kernels form b = re^2 + im^2 while staging a tile.
+ * A must not be NULL.  Everything else as tetra_dos.
+ */
+int tetra_dos_complex(tdos_plan* p, const float* E, const float* A, int layout, const float* omega, int nE,
+                      float* dos, float* nos, int memspace, void* cuda_stream);
+
+/*
  * Multi-GPU building blocks (device pointers only).
  * tetra_dos_partial: the additive share of the cubes with z_lo <= iz < z_hi, as raw fp64 sums
  *   part[3][norb][nE]  (0: sum b*dw/V, 1: sum b*w/V over E1 < omega < E4, 2: Eq.-15 step histogram / V at the first omega >= E4),

@@ -44,6 +44,7 @@ struct MainParams {
     int nmb;                     // orbital blocks of MB
     int n_items;                 // ntx*nty*ntz*nb*nmb
     int unitW;                   // W == 1
+    int cplx;                    // W holds complex eigenvector elements a (re, im pairs), strides count pairs: b = |a|^2
     int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
     float* partial;              // [gridDim.x] x { D[norb][nE], T[norb][nE], S[nE][norb] }
     unsigned int* next_item;        // tdos_main5: work counter, zero at launch
@@ -54,6 +55,15 @@ struct MainParams {
 // (dx,dy,dz) = bits 0,1,2 of c (reading G7).
 __device__ __constant__ int8_t kTableI[6][4] = {
     {0, 1, 2, 5}, {1, 2, 3, 5}, {0, 2, 4, 5}, {2, 3, 5, 7}, {2, 4, 5, 6}, {2, 5, 6, 7}};
+
+// b_{n,m}(k) = |a_n^m(k)|^2 (Eq. 3, :48; the paper ships re and im separately, :263) or the weight itself
+__device__ __forceinline__ float load_weight(const MainParams& p, long long idx) {
+    if (p.cplx) {
+        const float2 a = __ldg(reinterpret_cast<const float2*>(p.W) + idx);
+        return fmaf(a.x, a.x, a.y * a.y);
+    }
+    return __ldg(p.W + idx);
+}
 
 // first index i in [0, nE] with omega[i] >= x (STRICT = false) or omega[i] > x (STRICT = true):
 // direct index guess for a uniform grid, then an exact fix-up on the stored fp32 energies.
@@ -245,7 +255,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     }
     float* part = p.partial + (size_t)blockIdx.x * 3 * norb * nE;   // rows [bin][ D | T | S ]
     const bool vec4 = (MB % 4 == 0) && (norb % 4 == 0);          // 16-byte aligned vector reductions
-    const bool w_vec4 = (MB % 4 == 0) && !p.unitW && p.sWm == 1 && (norb % 4 == 0) &&
+    const bool w_vec4 = (MB % 4 == 0) && !p.unitW && !p.cplx && p.sWm == 1 && (norb % 4 == 0) &&
                         ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
 
     const int g = lane / GL, gl = lane % GL;
@@ -291,7 +301,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
-                sW[k * WST + m] = (m0 + m < norb) ? __ldg(p.W + ik * p.sWk + (long long)n * p.sWn + (m0 + m)) : 0.0f;
+                sW[k * WST + m] = (m0 + m < norb) ? load_weight(p, ik * p.sWk + (long long)n * p.sWn + (m0 + m)) : 0.0f;
             }
         } else {                   // k contiguous (SoA): k fastest across lanes
             for (int q = lane; q < PK * MB; q += 32) {
@@ -300,7 +310,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
                 sW[k * WST + m] = (m0 + m < norb)
-                                      ? __ldg(p.W + ik * p.sWk + (long long)n * p.sWn + (long long)(m0 + m) * p.sWm)
+                                      ? load_weight(p, ik * p.sWk + (long long)n * p.sWn + (long long)(m0 + m) * p.sWm)
                                       : 0.0f;
             }
         }

@@ -102,6 +102,8 @@ struct tdos_plan {
     // host-mode staging
     float* dE = nullptr;
     float* dW = nullptr;
+    size_t dW_floats = 0;         // capacity of dW
+    int cplx = 0;                 // the call in flight passes complex eigenvector elements instead of weights
     float* dOm = nullptr;
     float* dDos = nullptr;
     float* dNos = nullptr;
@@ -287,6 +289,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     if (items > 0x7fffffffLL) return TDOS_EINVAL;
     mp.n_items = (int)items;
     mp.unitW = (W == nullptr);
+    mp.cplx = (W != nullptr) ? p->cplx : 0;
     mp.partial = p->partial;
     mp.counters = p->counters;
     mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
@@ -383,8 +386,26 @@ static int run_device(tdos_plan* p, const float* E, const float* W, int layout, 
     return TDOS_OK;
 }
 
+static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+                          float* dos, float* nos, int memspace, void* cuda_stream);
+
 int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE, float* dos,
               float* nos, int memspace, void* cuda_stream) {
+    if (p) p->cplx = 0;
+    return tetra_dos_impl(p, E, W, layout, omega, nE, dos, nos, memspace, cuda_stream);
+}
+
+int tetra_dos_complex(tdos_plan* p, const float* E, const float* A, int layout, const float* omega, int nE,
+                      float* dos, float* nos, int memspace, void* cuda_stream) {
+    if (!p || !A) return TDOS_EINVAL;
+    p->cplx = 1;
+    const int rc = tetra_dos_impl(p, E, A, layout, omega, nE, dos, nos, memspace, cuda_stream);
+    p->cplx = 0;
+    return rc;
+}
+
+static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+                          float* dos, float* nos, int memspace, void* cuda_stream) {
     int rc = check_common(p, E, W, layout, omega, nE);
     if (rc) return rc;
     if (!dos) return TDOS_EINVAL;
@@ -397,14 +418,29 @@ int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const fl
         if (!(omega[i] > omega[i - 1])) return TDOS_EINVAL;
     const size_t nkt = (size_t)p->nk[0] * p->nk[1] * p->nk[2];
     const size_t nEb = (size_t)p->nE_max * sizeof(float);
+    const size_t wfl = (size_t)(p->cplx ? 2 : 1);   // floats per orbital weight as the caller passes them
+    if (p->dE && p->dW_floats < nkt * p->nb * p->norb * wfl) {   // a complex call after real ones: grow the staging buffer
+        cudaFree(p->dW);
+        p->dW = nullptr;
+        p->dW_floats = 0;
+        if (cudaMalloc(&p->dW, nkt * p->nb * p->norb * wfl * sizeof(float)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(p->dE); cudaFree(p->dOm); cudaFree(p->dDos); cudaFree(p->dNos);
+            p->dE = p->dOm = p->dDos = p->dNos = nullptr;
+            return TDOS_ENOMEM;
+        }
+        p->dW_floats = nkt * p->nb * p->norb * wfl;
+    }
     if (!p->dE) {
+        p->dW_floats = nkt * p->nb * p->norb * wfl;
         if (cudaMalloc(&p->dE, nkt * p->nb * sizeof(float)) != cudaSuccess ||
-            cudaMalloc(&p->dW, nkt * p->nb * p->norb * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&p->dW, p->dW_floats * sizeof(float)) != cudaSuccess ||
             cudaMalloc(&p->dOm, nEb) != cudaSuccess || cudaMalloc(&p->dDos, nEb * p->norb) != cudaSuccess ||
             cudaMalloc(&p->dNos, nEb * p->norb) != cudaSuccess) {
             cudaGetLastError();
             cudaFree(p->dE); cudaFree(p->dW); cudaFree(p->dOm); cudaFree(p->dDos); cudaFree(p->dNos);
             p->dE = p->dW = p->dOm = p->dDos = p->dNos = nullptr;
+            p->dW_floats = 0;
             return TDOS_ENOMEM;
         }
     }
@@ -415,7 +451,7 @@ int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const fl
     cudaStream_t st = p->main, cp = p->side;
     const int N3 = p->nk[2];
     const size_t plane = (size_t)p->nk[0] * p->nk[1];
-    const size_t total = nkt * p->nb * (1 + (W ? (size_t)p->norb : 0)) * sizeof(float);
+    const size_t total = nkt * p->nb * (1 + (W ? (size_t)p->norb * wfl : 0)) * sizeof(float);
     int nslab = (int)((total + kSlabBytes - 1) / kSlabBytes);
     if (nslab > tdos_plan::kMaxSlabs) nslab = tdos_plan::kMaxSlabs;
     if (nslab > N3) nslab = N3;
@@ -431,7 +467,7 @@ int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const fl
         if (c_hi > c_lo) {
             const size_t k0 = (size_t)c_lo * plane, nk_s = (size_t)(c_hi - c_lo) * plane;
             if (layout == TDOS_AOS) {
-                const size_t se = (size_t)p->nb, sw = (size_t)p->nb * p->norb;
+                const size_t se = (size_t)p->nb, sw = (size_t)p->nb * p->norb * wfl;
                 CK(cudaMemcpyAsync(p->dE + k0 * se, E + k0 * se, nk_s * se * sizeof(float), cudaMemcpyHostToDevice, cp));
                 if (W)
                     CK(cudaMemcpyAsync(p->dW + k0 * sw, W + k0 * sw, nk_s * sw * sizeof(float), cudaMemcpyHostToDevice, cp));
@@ -440,7 +476,7 @@ int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const fl
                 CK(cudaMemcpy2DAsync(p->dE + k0, pitch, E + k0, pitch, nk_s * sizeof(float), (size_t)p->nb,
                                      cudaMemcpyHostToDevice, cp));
                 if (W)
-                    CK(cudaMemcpy2DAsync(p->dW + k0, pitch, W + k0, pitch, nk_s * sizeof(float),
+                    CK(cudaMemcpy2DAsync(p->dW + k0 * wfl, pitch * wfl, W + k0 * wfl, pitch * wfl, nk_s * wfl * sizeof(float),
                                          (size_t)p->nb * p->norb, cudaMemcpyHostToDevice, cp));
             }
         }

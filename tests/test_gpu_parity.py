@@ -297,3 +297,38 @@ def test_generation5_edge_cases(nk, nb, norb, nE):
     ref2 = oracle.tetra_dos(E2, W, nk, om2)
     dos, nos = run_gpu(E2, W, nk, om2)
     assert_parity(ref2, dos, nos, "gen5 ties %s" % (nk,))
+
+
+@pytest.mark.parametrize("nk,nb,norb,nE", [((6, 5, 8), 2, 8, 300), ((5, 4, 3), 3, 3, 120)])
+def test_complex_eigenvector_input(nk, nb, norb, nE):
+    """tetra_dos_complex takes the eigenvector elements a_n^m(k) (re, im), as the paper's
+    kernel does, and squares them while staging; result = tetra_dos on b = abs(a)^2."""
+    import torch
+    E, W = wl.random_bands(nk, nb, norb, seed=41)
+    rng = np.random.default_rng(5)
+    phase = rng.uniform(0, 2 * np.pi, W.shape)
+    A = np.stack([np.sqrt(W) * np.cos(phase), np.sqrt(W) * np.sin(phase)], axis=-1).astype(np.float32)   # [ik][n][m][2]
+    Wb = (A[..., 0].astype(np.float64) ** 2 + A[..., 1].astype(np.float64) ** 2).astype(np.float32)
+    om = wl.omega_grid(-1.2, 1.3, nE)
+    ref = oracle.tetra_dos(E, Wb, nk, om)
+    dev = torch.device("cuda:0")
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        for layout in (binding.TDOS_AOS, binding.TDOS_SOA):
+            Ex = E if layout == binding.TDOS_AOS else np.ascontiguousarray(E.T)
+            Ax = A if layout == binding.TDOS_AOS else np.ascontiguousarray(A.transpose(1, 2, 0, 3))   # [n][m][ik][2]
+            dE, dA, dOm = (torch.from_numpy(np.ascontiguousarray(x)).to(dev) for x in (Ex, Ax, om))
+            dos = torch.full((norb, nE), float("nan"), device=dev)
+            nos = torch.full((norb, nE), float("nan"), device=dev)
+            plan.tetra_dos_complex(dE, dA, dOm, dos, nos, layout=layout)
+            torch.cuda.synchronize()
+            assert_parity(ref, dos.cpu().numpy(), nos.cpu().numpy(), "complex layout %d" % layout)
+            hdos = np.full((norb, nE), np.nan, dtype=np.float32)
+            hnos = np.full((norb, nE), np.nan, dtype=np.float32)
+            plan.tetra_dos_complex(Ex, Ax, om, hdos, hnos, layout=layout, memspace=binding.TDOS_HOST)
+            assert_parity(ref, hdos, hnos, "complex host layout %d" % layout)
+        # a real call on the same plan afterwards still works (the staging buffer only ever grows)
+        hdos = np.zeros((norb, nE), dtype=np.float32)
+        plan.tetra_dos(E, Wb, om, hdos, None, memspace=binding.TDOS_HOST)
+        assert_parity(ref, hdos, None, "real after complex")
+        with pytest.raises(binding.TdosError):
+            plan.tetra_dos_complex(E, None, om, hdos, None, memspace=binding.TDOS_HOST)
