@@ -36,6 +36,8 @@ def _load():
         lib.oracle_corner_weights.argtypes = [dp, C.c_double, C.c_double, dp, dp]
         lib.oracle_corner_weights.restype = C.c_int
         lib.oracle_sort4.argtypes = [dp, dp, ip]
+        lib.oracle_tetra_weights.argtypes = [fp, ip, C.c_int, C.c_int, fp, C.c_int, dp, dp]
+        lib.oracle_tetra_weights.restype = C.c_int
         lib.oracle_table_I.argtypes = [ip]
         lib.oracle_corner_offset.argtypes = [C.c_int, ip]
         lib.oracle_tetra_dos.argtypes = [fp, fp, ip, C.c_int, C.c_int, C.c_int, fp, C.c_int,
@@ -130,3 +132,20 @@ def tetra_dos(E, W, nk, omega, layout: int = AOS, windowed: bool = False, nthrea
         raise ValueError("oracle_tetra_dos: bad arguments (rc=%d)" % rc)
     return {"dos": dos, "nos": nos, "n_tb": int(cnt[0]), "n_eval": int(cnt[1]),
             "n_case": [int(x) for x in cnt[2:5]]}
+
+
+def tetra_weights(E, nk, energies, layout: int = AOS):
+    """Per-k-point integration weights of PAPER.md Eq. 5-7: returns (wk, dwk), each [nW][nb][nk] float64."""
+    lib = _load()
+    nk = tuple(int(x) for x in nk)
+    nkt = nk[0] * nk[1] * nk[2]
+    E = np.ascontiguousarray(E, dtype=np.float32)
+    nb = E.shape[1] if layout == AOS else E.shape[0]
+    en = np.ascontiguousarray(energies, dtype=np.float32)
+    wk = np.zeros((len(en), nb, nkt))
+    dwk = np.zeros((len(en), nb, nkt))
+    rc = lib.oracle_tetra_weights(E.ctypes.data_as(C.POINTER(C.c_float)), (C.c_int * 3)(*nk), nb, layout,
+                                  en.ctypes.data_as(C.POINTER(C.c_float)), len(en), _dptr(wk), _dptr(dwk))
+    if rc != 0:
+        raise ValueError("oracle_tetra_weights: bad arguments")
+    return wk, dwk

@@ -347,3 +347,52 @@ int oracle_max_threads(void) {
     return 1;
 #endif
 }
+
+/*
+ * Generic tetrahedron integration weights (Eq. 5-7, :58-71): for every k-point j and band n,
+ *     wk[e][n][j] = sum over the tetrahedra T that have j as a corner of w_{n,l(j,T)}(E_e),
+ * so that <X>(E_e) = sum_n sum_j X_n(k_j) wk[e][n][j] for any X (Eq. 7), and dwk the same with dw/dE
+ * (X = b_{n,m} gives N_m and DOS_m of oracle_tetra_dos: that identity is the pin of this routine's
+ * corner <-> k-point bookkeeping, tests/test_oracle_pins.py).  Same cubes, Table I, wrap, sort and
+ * test order as oracle_tetra_dos; strictly sequential; the literal Eq. 11-15 for every energy.
+ * wk, dwk: out [nW][nb][nk] doubles (k fastest), overwritten; dwk may be NULL.
+ */
+int oracle_tetra_weights(const float* E, const int nk3[3], int nb, int layout, const float* energies, int nW,
+                         double* wk, double* dwk) {
+    if (!E || !nk3 || !energies || !wk || nb < 1 || nW < 1) return -1;
+    const int N1 = nk3[0], N2 = nk3[1], N3 = nk3[2];
+    if (N1 < 1 || N2 < 1 || N3 < 1) return -1;
+    const long nk = (long)N1 * N2 * N3;
+    const double V = 1.0 / (24.0 * (double)nk); /* G9: V_T/(4 V_G) */
+    memset(wk, 0, sizeof(double) * (size_t)nW * nb * nk);
+    if (dwk) memset(dwk, 0, sizeof(double) * (size_t)nW * nb * nk);
+    for (long cube = 0; cube < nk; cube++) {
+        const int ix = (int)(cube % N1), iy = (int)((cube / N1) % N2), iz = (int)(cube / ((long)N1 * N2));
+        long corner[8];
+        for (int c = 1; c <= 8; c++) {
+            int d[3];
+            oracle_corner_offset(c, d);
+            corner[c - 1] = (long)((ix + d[0]) % N1) + (long)N1 * (((iy + d[1]) % N2) + (long)N2 * ((iz + d[2]) % N3));
+        }
+        for (int i = 0; i < 6; i++)
+            for (int n = 0; n < nb; n++) {
+                double e_in[4], e[4], w[4], dw[4];
+                int perm[4];
+                long kk[4];
+                for (int l = 0; l < 4; l++) {
+                    kk[l] = corner[TABLE_I[i][l] - 1];
+                    e_in[l] = get_E(E, layout, nk, nb, kk[l], n);
+                }
+                oracle_sort4(e_in, e, perm);
+                for (int q = 0; q < nW; q++) {
+                    oracle_corner_weights(e, (double)energies[q], V, w, dw);
+                    for (int l = 0; l < 4; l++) {
+                        const size_t o = ((size_t)q * nb + n) * nk + kk[perm[l]];
+                        wk[o] += w[l];
+                        if (dwk) dwk[o] += dw[l];
+                    }
+                }
+            }
+    }
+    return 0;
+}

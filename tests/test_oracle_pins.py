@@ -425,3 +425,25 @@ def test_flat_band_and_grid_outside_bands(oracle_lib):
     hi = oracle_lib.tetra_dos(E, W, nk, np.array([4.0, 5.0], dtype=np.float32), windowed=True)
     assert not lo["dos"].any() and not lo["nos"].any() and not hi["dos"].any()
     assert np.allclose(hi["nos"], W.astype(np.float64).sum(axis=(0, 1))[:, None] / n, atol=1e-13)
+
+
+def test_per_k_weights_reproduce_the_orbital_sums(oracle_lib):
+    """Pin of oracle.tetra_weights (Eq. 5-7): with X = b_{n,m} the per-k weights must give back
+    N_m and DOS_m of tetra_dos (Eq. 7 vs Eq. 8-9: the same sum in another order), which fixes the
+    corner <-> k-point bookkeeping; every k-point is a corner of 24 tetrahedra, so above all bands each weight
+    is 24 V = 1/nk (Eq. 15) and below all bands it is 0 (Eq. 11)."""
+    nk, nb, norb = (4, 3, 5), 3, 4
+    E, W = wl.random_bands(nk, nb, norb, seed=17)
+    om = np.array([-2.0, -0.6, -0.1, 0.05, 0.4, 0.9, 2.0], dtype=np.float32)
+    for layout in (oracle_lib.AOS, oracle_lib.SOA):
+        Ex = E if layout == oracle_lib.AOS else np.ascontiguousarray(E.T)
+        wk, dwk = oracle_lib.tetra_weights(Ex, nk, om, layout=layout)
+        ref = oracle_lib.tetra_dos(E, W, nk, om)
+        Wd = W.astype(np.float64)                                  # [k][n][m]
+        nos = np.einsum("enk,knm->me", wk, Wd)
+        dos = np.einsum("enk,knm->me", dwk, Wd)
+        assert np.allclose(nos, ref["nos"], rtol=1e-12, atol=1e-15)
+        assert np.allclose(dos, ref["dos"], rtol=1e-12, atol=1e-14)
+        assert not wk[0].any() and not dwk[0].any()
+        assert np.allclose(wk[-1], 1.0 / np.prod(nk), rtol=1e-13) and not dwk[-1].any()
+        assert (wk >= 0).all()
