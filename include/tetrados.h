@@ -127,6 +127,17 @@ int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, flo
                        void* cuda_stream);
 
 /*
+ * Generic tetrahedron integration weights (Eq. 5-7, :58-71): for nW energies (device array, any order)
+ *     wk[e][n][ik]  = sum over the tetrahedra with corner ik of w_{n,l}(energies[e])        (Eq. 11-15)
+ *     dwk[e][n][ik] = the same with dw/dE (may be NULL),
+ * both [nW][nb][nk] floats on the device, k fastest, overwritten, normalised so that
+ * <X>(E) = sum_n sum_ik X_n(k_ik) wk[e][n][ik] (Eq. 7); X = 1 gives the integrated DOS, X = b_{n,m} gives N_m.
+ * E in `layout` as for tetra_dos; the plan's norb is not used.  Asynchronous on `cuda_stream`.
+ */
+int tetra_weights(tdos_plan* p, const float* E, int layout, const float* energies, int nW, float* wk, float* dwk,
+                  void* cuda_stream);
+
+/*
  * One-shot convenience matching the paper's "called from a CPU code" scenario:
  * host pointers, AoS layout, cubic Nk^3 grid, omega_i = (float)(omega_min + i*(omega_max-omega_min)/(nE-1))
  * evaluated in double (endpoints inclusive).  Creates a plan on the current device,

@@ -17,7 +17,7 @@ TDOS_MAX_NE = 65534
 
 # every symbol include/tetrados.h declares
 SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy",
-           "tetra_dos", "tetra_dos_complex", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
+           "tetra_dos", "tetra_dos_complex", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
            "tdos_last_counters", "tdos_kernel_ms", "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
 
 _lib = None
@@ -51,6 +51,7 @@ def load():
     lib.tdos_plan_destroy.argtypes = [vp]
     lib.tetra_dos.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
     lib.tetra_dos_complex.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
+    lib.tetra_weights.argtypes = [vp, fp, C.c_int, fp, C.c_int, fp, fp, vp]
     lib.tetra_dos_partial.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, C.c_int, C.c_int, vp, vp]
     lib.tetra_dos_finalize.argtypes = [vp, vp, C.c_int, fp, fp, vp]
     lib.tetra_dos_simple.argtypes = [fp, fp, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_int, fp, fp]
@@ -124,6 +125,11 @@ class Plan:
         nE = int(omega.shape[0])
         _check(load().tetra_dos_complex(self._h, _ptr(E), _ptr(A), layout, _ptr(omega), nE, _ptr(dos), _ptr(nos),
                                         memspace, _stream_ptr(stream, memspace)), "tetra_dos_complex")
+
+    def tetra_weights(self, E, energies, wk, dwk=None, layout: int = TDOS_AOS, stream=None):
+        """tetra_weights(): per-k-point integration weights wk[nW][nb][nk] (and dwk) for device tensors."""
+        _check(load().tetra_weights(self._h, _ptr(E), layout, _ptr(energies), int(energies.shape[0]), _ptr(wk), _ptr(dwk),
+                                    _stream_ptr(stream, TDOS_DEVICE)), "tetra_weights")
 
     def tetra_dos_partial(self, E, W, omega, z_lo: int, z_hi: int, part, layout: int = TDOS_AOS, stream=None):
         nE = int(omega.shape[0])

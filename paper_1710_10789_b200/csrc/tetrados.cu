@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "tdos_kernels.cuh"
+#include "tdos_kweights.cuh"
 #include "tdos_main5.cuh"
 
 namespace {
@@ -496,6 +497,33 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
     CK(cudaMemcpyAsync(dos, p->dDos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
     if (nos) CK(cudaMemcpyAsync(nos, p->dNos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return TDOS_OK;
+}
+
+int tetra_weights(tdos_plan* p, const float* E, int layout, const float* energies, int nW, float* wk, float* dwk,
+                  void* cuda_stream) {
+    if (!p || !E || !energies || !wk || nW < 1) return TDOS_EINVAL;
+    if (layout != TDOS_AOS && layout != TDOS_SOA) return TDOS_EINVAL;
+    CK(cudaSetDevice(p->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long nkt = (long long)p->nk[0] * p->nk[1] * p->nk[2];
+    tdos::KWeightParams kp{};
+    kp.E = E;
+    kp.energies = energies;
+    if (layout == TDOS_AOS) { kp.sEk = p->nb; kp.sEn = 1; } else { kp.sEk = 1; kp.sEn = nkt; }
+    kp.N1 = p->nk[0]; kp.N2 = p->nk[1]; kp.N3 = p->nk[2];
+    kp.nb = p->nb; kp.nW = nW;
+    kp.V = (float)(1.0 / (24.0 * (double)nkt));
+    kp.wk = wk;
+    kp.dwk = dwk;
+    const size_t bytes = (size_t)nW * p->nb * nkt * sizeof(float);
+    CK(cudaMemsetAsync(wk, 0, bytes, st));
+    if (dwk) CK(cudaMemsetAsync(dwk, 0, bytes, st));
+    const long long total = nkt * 6 * p->nb;
+    long long blocks = (total + 255) / 256;
+    if (blocks > (long long)p->num_sms * 32) blocks = (long long)p->num_sms * 32;
+    tdos::tdos_kweights<<<(int)blocks, 256, 0, st>>>(kp);
+    CK(cudaGetLastError());
     return TDOS_OK;
 }
 

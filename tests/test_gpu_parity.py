@@ -332,3 +332,32 @@ def test_complex_eigenvector_input(nk, nb, norb, nE):
         assert_parity(ref, hdos, None, "real after complex")
         with pytest.raises(binding.TdosError):
             plan.tetra_dos_complex(E, None, om, hdos, None, memspace=binding.TDOS_HOST)
+
+
+@pytest.mark.parametrize("nk,nb", [((6, 5, 4), 3), ((2, 2, 2), 1), ((9, 7, 5), 2)])
+def test_per_k_integration_weights(nk, nb):
+    """tetra_weights (Eq. 5-7) against oracle.tetra_weights, element by element; odd and
+    even numbers of energies, an energy below and above all bands, energies ON band values (ties, G10)."""
+    import torch
+    E, _ = wl.random_bands(nk, nb, 1, seed=23)
+    n = int(np.prod(nk))
+    en = np.array([-2.0, -0.7, -0.2, float(E[0, 0]), 0.1, 0.55, 3.0], dtype=np.float32)
+    dev = torch.device("cuda:0")
+    with binding.Plan(nk, nb, 1, 8) as plan:
+        for nW in (7, 4, 1):
+            for layout in (binding.TDOS_AOS, binding.TDOS_SOA):
+                Ex = E if layout == binding.TDOS_AOS else np.ascontiguousarray(E.T)
+                wk_ref, dwk_ref = oracle.tetra_weights(Ex, nk, en[:nW], layout=layout)
+                dE, dEn = torch.from_numpy(np.ascontiguousarray(Ex)).to(dev), torch.from_numpy(en[:nW].copy()).to(dev)
+                wk = torch.full((nW, nb, n), float("nan"), device=dev)
+                dwk = torch.full((nW, nb, n), float("nan"), device=dev)
+                plan.tetra_weights(dE, dEn, wk, dwk, layout=layout)
+                torch.cuda.synchronize()
+                w, d = wk.cpu().numpy().astype(np.float64), dwk.cpu().numpy().astype(np.float64)
+                assert np.abs(w - wk_ref).max() <= 5e-6 / n, np.abs(w - wk_ref).max() * n
+                assert np.abs(d - dwk_ref).max() <= 1e-5 * max(np.abs(dwk_ref).max(), 1e-300)
+                assert not w[wk_ref == 0].any()
+                wk2 = torch.full((nW, nb, n), float("nan"), device=dev)
+                plan.tetra_weights(dE, dEn, wk2, None, layout=layout)        # dwk = NULL
+                torch.cuda.synchronize()
+                assert torch.equal(torch.nan_to_num(wk2), torch.nan_to_num(wk)) or np.allclose(wk2.cpu().numpy(), w, atol=1e-6 / n)
