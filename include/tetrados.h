@@ -27,7 +27,9 @@
  *
  * Kernels: tdos_main5 (one record per interval of Eq. 12-14; norb >= 5 and norb % 4 == 0) or tdos_main (any norb);
  * the environment variables TDOS_KERNEL=3|5 and TDOS_TILE=<index>, read at plan creation, override the choice of
- * kernel and tile shape for experiments.
+ * kernel and tile shape for experiments.  Without TDOS_KERNEL a plan that started with
+ * tdos_main5 reads the work counters of its first call when the second call starts (one host-side wait for the
+ * first call's kernel) and keeps tdos_main from then on if the windows average fewer than 6 energies.
  *
  * Ownership: the caller owns every array; the library never frees them and does not retain them
  * past the call (device mode: past completion of the work queued on `stream`).  A plan owns all

@@ -20,6 +20,9 @@ namespace {
 
 thread_local char g_cuda_err[256] = "";
 
+// mean number of bins with E1 < omega < E4 per (tetrahedron, band) below which generation 3 is used
+constexpr double kShortWindowBins = 6.0;
+
 // host mode: bytes of E + W per staged z-slab (copy/compute overlap granularity)
 constexpr size_t kSlabBytes = (size_t)64 << 20;
 
@@ -94,7 +97,11 @@ struct tdos_plan {
     int nb = 0, norb = 0, nE_max = 0;
     int num_sms = 0;
     size_t smem_optin = 0;        // cudaDevAttrMaxSharedMemoryPerBlockOptin
-    Variant var{};
+    Variant var{};                // the main kernel in use
+    Variant var_short{};          // generation 3: better when the windows are a few bins only
+    int adapt = 0;                // 0: fixed; 1: first call done with generation 5, choice pending; 2: decided
+    unsigned long long* h_stat = nullptr;   // pinned copy of {n_tb, n_eval} of the first call
+    cudaEvent_t stat_ev = nullptr;
     int blocks_per_sm = 0;
     int grid = 0;
     float* partial = nullptr;     // [grid][3][norb][nE_max]
@@ -158,6 +165,8 @@ int tdos_plan_destroy(tdos_plan* p) {
         if (e) cudaEventDestroy(e);
     for (auto& e : p->cp_ev)
         if (e) cudaEventDestroy(e);
+    if (p->stat_ev) cudaEventDestroy(p->stat_ev);
+    if (p->h_stat) cudaFreeHost(p->h_stat);
     for (auto& tr : p->ring)
         for (auto& e : tr)
             if (e) cudaEventDestroy(e);
@@ -213,6 +222,20 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
         delete p;
         return rc;
     }
+    // Without TDOS_KERNEL the plan looks at the work counters of its first call: with windows of a few bins only
+    // (config 5: 3 bins on average) the three-records-per-tetrahedron scheme of generation 5 costs more than it saves.
+    if (gen == 5 && !kv) {
+        p->var_short = variants(8)[0];
+        int bps = 0;
+        if (cudaFuncSetAttribute((const void*)p->var_short.fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)p->var_short.smem) == cudaSuccess &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)p->var_short.fn, p->var_short.NWARP * 32,
+                                                          p->var_short.smem) == cudaSuccess &&
+            bps == p->blocks_per_sm && cudaMallocHost(&p->h_stat, 2 * sizeof(unsigned long long)) == cudaSuccess &&
+            cudaEventCreateWithFlags(&p->stat_ev, cudaEventDisableTiming) == cudaSuccess)
+            p->adapt = -1;   // armed: becomes 1 after the first call
+        cudaGetLastError();
+    }
     if (const char* s = getenv("TDOS_BLOCKS_PER_SM")) {
         int b = atoi(s);
         if (b >= 1 && b < p->blocks_per_sm) p->blocks_per_sm = b;
@@ -265,6 +288,11 @@ static int rows_per_block(const tdos_plan* p, int nE) { return p->var.gen == 5 ?
 // work counters (a call may cover the grid with several slab launches that accumulate into the same partials)
 static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
                         int z_lo, int z_hi, bool first, cudaStream_t st) {
+    if (first && p->adapt == 1) {   // second call: the first one's counters decide, once and for the plan's lifetime
+        CK(cudaEventSynchronize(p->stat_ev));
+        if (p->h_stat[0] > 0 && (double)p->h_stat[1] < kShortWindowBins * (double)p->h_stat[0]) p->var = p->var_short;
+        p->adapt = 2;
+    }
     const Variant& v = p->var;
     const long long nkt = (long long)p->nk[0] * p->nk[1] * p->nk[2];
     MainParams mp{};
@@ -332,6 +360,11 @@ static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st
     tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->grid, p->norb, nE, rows_per_block(p, nE), part_out);
     CK(cudaGetLastError());
     p->last_launches += 1;
+    if (p->adapt == -1) {   // first call of an adaptive plan: keep its work counters for the choice of kernel
+        CK(cudaMemcpyAsync(p->h_stat, p->counters, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CK(cudaEventRecord(p->stat_ev, st));
+        p->adapt = 1;
+    }
     return TDOS_OK;
 }
 
