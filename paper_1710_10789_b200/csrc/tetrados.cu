@@ -25,6 +25,8 @@ constexpr double kShortWindowBins = 6.0;
 
 // host mode: bytes of E + W per staged z-slab (copy/compute overlap granularity)
 constexpr size_t kSlabBytes = (size_t)64 << 20;
+// the first slabs are smaller (8 MB, doubling): the kernels start after 0.15 ms of copying instead of 1.2 ms
+constexpr size_t kFirstSlabBytes = (size_t)8 << 20;
 
 int cuda_fail(cudaError_t e, const char* what) {
     snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
@@ -486,17 +488,42 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
     const int N3 = p->nk[2];
     const size_t plane = (size_t)p->nk[0] * p->nk[1];
     const size_t total = nkt * p->nb * (1 + (W ? (size_t)p->norb * wfl : 0)) * sizeof(float);
-    int nslab = (int)((total + kSlabBytes - 1) / kSlabBytes);
-    if (nslab > tdos_plan::kMaxSlabs) nslab = tdos_plan::kMaxSlabs;
-    if (nslab > N3) nslab = N3;
-    if (nslab < 1) nslab = 1;
+    // slab boundaries zb[0..nslab]: 8, 16, 32 MB, then 64 MB each, then 32, 16, 8 MB -- a short first slab lets the
+    // kernels start early (compute-bound case), a short last one leaves little to compute after the last copy
+    // (copy-bound case)
+    int zb[tdos_plan::kMaxSlabs + 1];
+    int nslab = 0;
+    {
+        const double plane_bytes = (double)total / (double)N3;
+        const double ramp = 7.0 * (double)kFirstSlabBytes;                     // 8 + 16 + 32 MB
+        int nmid = (int)(((double)total - 2.0 * ramp) / (double)kSlabBytes + 0.999);
+        if (nmid < 0) nmid = 0;
+        if (nmid > tdos_plan::kMaxSlabs - 6) nmid = tdos_plan::kMaxSlabs - 6;
+        const double covered = 2.0 * ramp + (double)nmid * (double)kSlabBytes;
+        const double scale = (double)total > covered ? (double)total / covered : 1.0;
+        double sizes[tdos_plan::kMaxSlabs];
+        int ns = 0;
+        for (int i = 0; i < 3; i++) sizes[ns++] = (double)(kFirstSlabBytes << i);
+        for (int i = 0; i < nmid; i++) sizes[ns++] = (double)kSlabBytes;
+        for (int i = 2; i >= 0; i--) sizes[ns++] = (double)(kFirstSlabBytes << i);
+        zb[0] = 0;
+        double acc = 0.0;
+        for (int i = 0; i < ns && zb[nslab] < N3; i++) {
+            acc += sizes[i] * scale;
+            int z = (int)(acc / plane_bytes + 0.5);
+            if (z <= zb[nslab]) z = zb[nslab] + 1;
+            if (z > N3 || i == ns - 1) z = N3;
+            zb[++nslab] = z;
+        }
+        if (zb[nslab] < N3) zb[nslab] = N3;
+    }
     for (int i = 0; i < nslab; i++)
         if (!p->cp_ev[i]) CK(cudaEventCreateWithFlags(&p->cp_ev[i], cudaEventDisableTiming));
     CK(cudaMemcpyAsync(p->dOm, omega, (size_t)nE * sizeof(float), cudaMemcpyHostToDevice, st));
     p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
     CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
     for (int sidx = 0; sidx < nslab; sidx++) {
-        const int z_lo = (int)((long long)N3 * sidx / nslab), z_hi = (int)((long long)N3 * (sidx + 1) / nslab);
+        const int z_lo = zb[sidx], z_hi = zb[sidx + 1];
         const int c_lo = sidx == 0 ? 0 : z_lo + 1, c_hi = (z_hi + 1 < N3) ? z_hi + 1 : N3;
         if (c_hi > c_lo) {
             const size_t k0 = (size_t)c_lo * plane, nk_s = (size_t)(c_hi - c_lo) * plane;

@@ -361,3 +361,26 @@ def test_per_k_integration_weights(nk, nb):
                 plan.tetra_weights(dE, dEn, wk2, None, layout=layout)        # dwk = NULL
                 torch.cuda.synchronize()
                 assert torch.equal(torch.nan_to_num(wk2), torch.nan_to_num(wk)) or np.allclose(wk2.cpu().numpy(), w, atol=1e-6 / n)
+
+
+def test_plan_switches_kernel_for_short_windows(monkeypatch):
+    """Unless TDOS_KERNEL is set, a plan that started with tdos_main5 keeps tdos_main from its second call on when
+    the first call's counters show windows below 6 bins on average; results stay within tolerance either way."""
+    monkeypatch.delenv("TDOS_KERNEL", raising=False)
+    nk, nb, norb = (8, 8, 8), 2, 8
+    E, W = wl.tb8_bands(nk, threads=1)
+    E, W = np.ascontiguousarray(E[:, :nb]), np.ascontiguousarray(W[:, :nb, :])
+    for nE, expect in ((24, 3), (900, 5)):       # coarse grid: windows of about one bin; fine grid: tens of bins
+        om = wl.omega_grid(-6.0, 4.0, nE)
+        ref = oracle.tetra_dos(E, W, nk, om)
+        with binding.Plan(nk, nb, norb, nE) as plan:
+            for call in range(3):
+                dos, nos = run_gpu(E, W, nk, om, plan=plan)
+                assert_parity(ref, dos, nos, "adaptive nE %d call %d" % (nE, call))
+                assert plan.last_counters()["kernel"] == (5 if call == 0 else expect)
+    monkeypatch.setenv("TDOS_KERNEL", "5")
+    om = wl.omega_grid(-6.0, 4.0, 24)
+    with binding.Plan(nk, nb, norb, 24) as plan:
+        for call in range(2):
+            run_gpu(E, W, nk, om, plan=plan)
+            assert plan.last_counters()["kernel"] == 5
