@@ -46,7 +46,8 @@ struct MainParams {
     int unitW;                   // W == 1
     int cplx;                    // W holds complex eigenvector elements a (re, im pairs), strides count pairs: b = |a|^2
     int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
-    float* partial;              // [gridDim.x] x { D[norb][nE], T[norb][nE], S[nE][norb] }
+    int nparts;                  // tdos_main6: copies of the partial histogram (block b adds to copy b % nparts)
+    float* partial;              // [copies] x rows [nEp][ D(norb) | T(norb) | S(norb) ]; tdos_main, tdos_main5: one copy per block
     unsigned int* next_item;        // tdos_main5: work counter, zero at launch
     unsigned long long* counters;   // [0] n_tb, [1] n_eval = #(tb, omega) with E1 < omega < E4
 };

@@ -15,13 +15,11 @@
 #include "tdos_kernels.cuh"
 #include "tdos_kweights.cuh"
 #include "tdos_main5.cuh"
+#include "tdos_main6.cuh"
 
 namespace {
 
 thread_local char g_cuda_err[256] = "";
-
-// mean number of bins with E1 < omega < E4 per (tetrahedron, band) below which generation 3 is used
-constexpr double kShortWindowBins = 6.0;
 
 // host mode: bytes of E + W per staged z-slab (copy/compute overlap granularity)
 constexpr size_t kSlabBytes = (size_t)64 << 20;
@@ -43,11 +41,29 @@ using tdos::MainParams;
 typedef void (*main_kernel_t)(const MainParams);
 
 struct Variant {
-    main_kernel_t fn;      // tdos_main (generation 3) or tdos_main5 (generation 5)
+    main_kernel_t fn;      // tdos_main (generation 3), tdos_main5 (generation 5) or tdos_main6 (generation 6)
     int MB, TX, TY, TZ, GL, NWARP;
     size_t smem;
-    int gen = 3;                    // main kernel generation: 3 or 5
+    int gen = 3;                    // main kernel generation: 3, 5 or 6
+    int bps = 0;                    // generation 6: blocks per SM the kernel is built for
 };
+
+template <int TX, int TY, int TZ, int NWARP, int NORB, int BPS>
+Variant make_variant6() {
+    Variant v{tdos::tdos_main6<TX, TY, TZ, NWARP, NORB, BPS>, 8, TX, TY, TZ, 2, NWARP, tdos::Cfg6<TX, TY, TZ, NWARP>::bytes};
+    v.gen = 6;
+    v.bps = BPS;
+    return v;
+}
+
+// v6 configurations compiled in (TDOS_TILE=<index> selects another one for experiments)
+template <int NORB>
+std::vector<Variant> variants6() {
+    return {make_variant6<2, 4, 8, 8, NORB, 2>(), make_variant6<4, 4, 4, 8, NORB, 2>(), make_variant6<2, 2, 16, 8, NORB, 2>(),
+            make_variant6<4, 4, 8, 16, NORB, 1>(), make_variant6<2, 2, 8, 8, NORB, 2>(), make_variant6<2, 2, 8, 4, NORB, 4>(),
+            make_variant6<2, 4, 4, 4, NORB, 4>(), make_variant6<2, 2, 8, 6, NORB, 3>(), make_variant6<2, 4, 8, 12, NORB, 1>(),
+            make_variant6<2, 2, 8, 8, NORB, 3>(), make_variant6<2, 2, 8, 6, NORB, 4>(), make_variant6<2, 2, 8, 4, NORB, 6>()};
+}
 
 template <int TX, int TY, int TZ, int NWARP, int NORB>
 Variant make_variant5() {
@@ -99,14 +115,12 @@ struct tdos_plan {
     int nb = 0, norb = 0, nE_max = 0;
     int num_sms = 0;
     size_t smem_optin = 0;        // cudaDevAttrMaxSharedMemoryPerBlockOptin
+    size_t smem_per_sm = 0;       // cudaDevAttrMaxSharedMemoryPerMultiprocessor
     Variant var{};                // the main kernel in use
-    Variant var_short{};          // generation 3: better when the windows are a few bins only
-    int adapt = 0;                // 0: fixed; 1: first call done with generation 5, choice pending; 2: decided
-    unsigned long long* h_stat = nullptr;   // pinned copy of {n_tb, n_eval} of the first call
-    cudaEvent_t stat_ev = nullptr;
     int blocks_per_sm = 0;
     int grid = 0;
-    float* partial = nullptr;     // [grid][3][norb][nE_max]
+    int nparts = 0;               // copies of the partial histogram (generation 6: one per SM; else one per block)
+    float* partial = nullptr;     // [nparts] rows [nE_max + 3][3 * norb]
     double* part64 = nullptr;     // [3][norb][nE_max]
     unsigned long long* counters = nullptr;   // [2] n_tb, n_eval of the last call
     // host-mode staging
@@ -167,8 +181,6 @@ int tdos_plan_destroy(tdos_plan* p) {
         if (e) cudaEventDestroy(e);
     for (auto& e : p->cp_ev)
         if (e) cudaEventDestroy(e);
-    if (p->stat_ev) cudaEventDestroy(p->stat_ev);
-    if (p->h_stat) cudaFreeHost(p->h_stat);
     for (auto& tr : p->ring)
         for (auto& e : tr)
             if (e) cudaEventDestroy(e);
@@ -196,27 +208,30 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     p->nE_max = nE_max;
     p->num_sms = prop.multiProcessorCount;
     p->smem_optin = prop.sharedMemPerBlockOptin;
+    p->smem_per_sm = prop.sharedMemPerMultiprocessor;
 
     const char* kv = getenv("TDOS_KERNEL");
-    // generation 5 needs blocks of 8 orbitals to pay off; narrower problems use generation 3
+    // generations 5 and 6 work on blocks of 8 orbitals with 16-byte vector reductions; narrower problems use generation 3
     int gen = kv ? atoi(kv) : 5;
-    if (gen == 5 && (norb < 5 || norb % 4 != 0)) gen = 3;   // tdos_main5: blocks of 8 orbitals, 16-byte vector reductions
-    std::vector<Variant> vs = gen == 5 ? (norb == 8 ? variants5<8>() : variants5<0>()) : variants(pick_mb(norb));
+    if (gen != 3 && gen != 5 && gen != 6) gen = 5;
+    if (gen != 3 && (norb < 5 || norb % 4 != 0)) gen = 3;
+    std::vector<Variant> vs = gen == 6   ? (norb == 8 ? variants6<8>() : variants6<0>())
+                              : gen == 5 ? (norb == 8 ? variants5<8>() : variants5<0>())
+                                         : variants(pick_mb(norb));
     int sel = 0;
     // Tile shape of generation 5.  A tile whose bands span few energy bins keeps more (record, chunk) entries per
     // chunk.  The paper's workloads are layered materials sampled on grids like 60 x 60 x 10, with
     // the weak dispersion along z, so the default tile is long in z whenever the grid divides evenly (2 x 2 x 8
-    // cubes, 15.1 ms on config 4 against 15.7 ms for 4 x 4 x 2); TDOS_TILE=<index> overrides it.
+    // cubes); TDOS_TILE=<index> overrides it.
     if (gen == 5 && nk[2] % 8 == 0 && nk[0] % 2 == 0 && nk[1] % 2 == 0) sel = 1;
     if (const char* s = getenv("TDOS_TILE")) sel = atoi(s);
     if (sel < 0 || sel >= (int)vs.size()) sel = 0;
     p->var = vs[sel];
 
+    // The attribute belongs to the kernel function, not to the plan: always the device maximum, so that plans with
+    // different nE_max never lower each other's limit.
     const void* kfn = (const void*)p->var.fn;
-    size_t smem_attr = p->var.smem;
-    if (p->var.gen == 5 && p->var.smem + (size_t)nE_max * sizeof(float) <= p->smem_optin)
-        smem_attr += (size_t)nE_max * sizeof(float);
-    cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_attr);
+    cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_optin);
     if (e == cudaSuccess)
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->blocks_per_sm, kfn, p->var.NWARP * 32, p->var.smem);
     if (e != cudaSuccess || p->blocks_per_sm < 1) {
@@ -224,30 +239,18 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
         delete p;
         return rc;
     }
-    // Without TDOS_KERNEL the plan looks at the work counters of its first call: with windows of a few bins only
-    // (config 5: 3 bins on average) the three-records-per-tetrahedron scheme of generation 5 costs more than it saves.
-    if (gen == 5 && !kv) {
-        p->var_short = variants(8)[0];
-        int bps = 0;
-        if (cudaFuncSetAttribute((const void*)p->var_short.fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)p->var_short.smem) == cudaSuccess &&
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)p->var_short.fn, p->var_short.NWARP * 32,
-                                                          p->var_short.smem) == cudaSuccess &&
-            bps == p->blocks_per_sm && cudaMallocHost(&p->h_stat, 2 * sizeof(unsigned long long)) == cudaSuccess &&
-            cudaEventCreateWithFlags(&p->stat_ev, cudaEventDisableTiming) == cudaSuccess)
-            p->adapt = -1;   // armed: becomes 1 after the first call
-        cudaGetLastError();
-    }
+    if (p->var.gen == 6 && p->blocks_per_sm > p->var.bps) p->blocks_per_sm = p->var.bps;
     if (const char* s = getenv("TDOS_BLOCKS_PER_SM")) {
         int b = atoi(s);
         if (b >= 1 && b < p->blocks_per_sm) p->blocks_per_sm = b;
     }
     p->grid = p->num_sms * p->blocks_per_sm;
+    p->nparts = p->var.gen == 6 ? p->num_sms : p->grid;
 
     const size_t hist = (size_t)3 * norb * ((size_t)nE_max + 3);
-    if (cudaMalloc(&p->partial, hist * p->grid * sizeof(float)) != cudaSuccess ||
+    if (cudaMalloc(&p->partial, hist * p->nparts * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&p->part64, hist * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&p->counters, 4 * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaMalloc(&p->counters, 40 * sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError();
         tdos_plan_destroy(p);
         return TDOS_ENOMEM;
@@ -284,17 +287,12 @@ static int check_common(const tdos_plan* p, const float* E, const float* W, int 
 }
 
 // rows of one block's partial histogram: generation 5 flushes whole chunks of 4 bins
-static int rows_per_block(const tdos_plan* p, int nE) { return p->var.gen == 5 ? (nE + 3) & ~3 : nE; }
+static int rows_per_block(const tdos_plan* p, int nE) { return p->var.gen >= 5 ? (nE + 3) & ~3 : nE; }
 
 // enqueue the main kernel for the cube slab [z_lo, z_hi); `first` also clears the block partials and the
 // work counters (a call may cover the grid with several slab launches that accumulate into the same partials)
 static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
                         int z_lo, int z_hi, bool first, cudaStream_t st) {
-    if (first && p->adapt == 1) {   // second call: the first one's counters decide, once and for the plan's lifetime
-        CK(cudaEventSynchronize(p->stat_ev));
-        if (p->h_stat[0] > 0 && (double)p->h_stat[1] < kShortWindowBins * (double)p->h_stat[0]) p->var = p->var_short;
-        p->adapt = 2;
-    }
     const Variant& v = p->var;
     const long long nkt = (long long)p->nk[0] * p->nk[1] * p->nk[2];
     MainParams mp{};
@@ -322,27 +320,35 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     mp.unitW = (W == nullptr);
     mp.cplx = (W != nullptr) ? p->cplx : 0;
     mp.partial = p->partial;
+    mp.nparts = p->nparts;
     mp.counters = p->counters;
     mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
 
     const long long work = items;
-    // generation 5: a block-wide copy of omega in shared memory if the device limit allows it
+    // generations 5 and 6: a block-wide copy of omega in shared memory if it fits (generation 6: without costing a
+    // resident block)
     size_t smem = v.smem;
-    if (v.gen == 5 && v.smem + (size_t)nE * sizeof(float) <= p->smem_optin) {
+    const size_t om_bytes = (size_t)nE * sizeof(float);
+    if (v.gen == 5 && v.smem + om_bytes <= p->smem_optin) {
         mp.om_smem = 1;
-        smem += (size_t)nE * sizeof(float);
+        smem += om_bytes;
+    }
+    if (v.gen == 6 && v.smem + om_bytes <= p->smem_optin &&
+        (size_t)p->blocks_per_sm * (v.smem + om_bytes + 1024) <= p->smem_per_sm) {
+        mp.om_smem = 1;
+        smem += om_bytes;
     }
     const size_t hist = (size_t)3 * p->norb * mp.nEp;
     if (first) {
-        CK(cudaMemsetAsync(p->partial, 0, hist * p->grid * sizeof(float), st));
-        CK(cudaMemsetAsync(p->counters, 0, 4 * sizeof(unsigned long long), st));
+        CK(cudaMemsetAsync(p->partial, 0, hist * p->nparts * sizeof(float), st));
+        CK(cudaMemsetAsync(p->counters, 0, 40 * sizeof(unsigned long long), st));
         p->last_items = 0;
         p->last_launches = 0;
-    } else if (v.gen == 5) {
+    } else if (v.gen >= 5) {
         CK(cudaMemsetAsync(p->counters + 3, 0, sizeof(unsigned long long), st));
     }
     if (work > 0) {
-        const long long blocks_needed = (work + v.NWARP - 1) / v.NWARP;
+        const long long blocks_needed = v.gen == 6 ? work : (work + v.NWARP - 1) / v.NWARP;
         const int grid = (int)((blocks_needed < p->grid) ? blocks_needed : p->grid);
         v.fn<<<grid, v.NWARP * 32, smem, st>>>(mp);
         CK(cudaGetLastError());
@@ -359,14 +365,9 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
 static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st) {
     const size_t hist = (size_t)3 * p->norb * nE;
     const int mblocks = (int)((hist + 255) / 256);
-    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->grid, p->norb, nE, rows_per_block(p, nE), part_out);
+    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->nparts, p->norb, nE, rows_per_block(p, nE), part_out);
     CK(cudaGetLastError());
     p->last_launches += 1;
-    if (p->adapt == -1) {   // first call of an adaptive plan: keep its work counters for the choice of kernel
-        CK(cudaMemcpyAsync(p->h_stat, p->counters, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
-        CK(cudaEventRecord(p->stat_ev, st));
-        p->adapt = 1;
-    }
     return TDOS_OK;
 }
 
@@ -628,11 +629,22 @@ int tdos_last_counters(tdos_plan* p, long long cnt[4]) {
     if (!p || !cnt || !p->last_stream_valid) return TDOS_EINVAL;
     CK(cudaSetDevice(p->device));
     CK(cudaStreamSynchronize(p->last_stream));
+#ifdef TDOS_PHASES
+    {
+        unsigned long long ph[24];
+        CK(cudaMemcpy(ph, p->counters + 8, sizeof(ph), cudaMemcpyDeviceToHost));
+        for (int w = 0; w < 2; w++) {
+            fprintf(stderr, "phases (%s warp, kcycles per block):", w ? "last" : "first");
+            for (int k = 0; k < 12; k++) fprintf(stderr, " %.0f", (double)ph[12 * w + k] / p->grid / 1e3);
+            fprintf(stderr, "\n");
+        }
+    }
+#endif
     unsigned long long h[3];
     CK(cudaMemcpy(h, p->counters, sizeof(h), cudaMemcpyDeviceToHost));
     cnt[0] = (long long)h[0];
     cnt[1] = (long long)h[1];
-    cnt[2] = p->var.gen == 5 ? (long long)h[2] : -1;
+    cnt[2] = p->var.gen >= 5 ? (long long)h[2] : -1;
     cnt[3] = p->var.gen;
     return TDOS_OK;
 }
