@@ -46,11 +46,20 @@ struct MainParams {
     int unitW;                   // W == 1
     int cplx;                    // W holds complex eigenvector elements a (re, im pairs), strides count pairs: b = |a|^2
     int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
-    int nparts;                  // tdos_main6: copies of the partial histogram (block b adds to copy b % nparts)
-    float* partial;              // [copies] x rows [nEp][ D(norb) | T(norb) | S(norb) ]; tdos_main, tdos_main5: one copy per block
+    // kernel choice on the device (null: this kernel runs): {sum of window lengths in bins, (tetrahedron, band) pairs}
+    // of a sample, written by tdos_estimate earlier on the stream; see wanted_generation()
+    const unsigned long long* est;
+    float* partial;              // [gridDim.x] rows [nEp][ D(norb) | T(norb) | S(norb) ]
     unsigned int* next_item;        // tdos_main5: work counter, zero at launch
     unsigned long long* counters;   // [0] n_tb, [1] n_eval = #(tb, omega) with E1 < omega < E4
 };
+
+// Mean number of bins with E1 < omega < E4 per (tetrahedron, band) below which tdos_main (generation 3: one record per
+// tetrahedron) beats tdos_main5 (generation 5: one record per interval of Eq. 12-14) -- config 5's windows are 3 bins.
+constexpr unsigned long long kShortWindowBins = 6;
+__host__ __device__ __forceinline__ int wanted_generation(unsigned long long sum_bins, unsigned long long n_tb) {
+    return (n_tb > 0 && sum_bins < kShortWindowBins * n_tb) ? 3 : 5;
+}
 
 // Table I of the paper, corner labels 1..8 -> 0..7; label c sits at offset
 // (dx,dy,dz) = bits 0,1,2 of c (reading G7).
@@ -245,6 +254,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     int* sOff = reinterpret_cast<int*>(base + Cfg::off_off);
     uint32_t* sWm = reinterpret_cast<uint32_t*>(sOff + NCH);
 
+    if (p.est && wanted_generation(p.est[0], p.est[1]) != 3) return;   // the other kernel of the pair runs
     const int nE = p.nE;
     const int norb = p.norb;
     const float* __restrict__ omega = p.omega;
@@ -254,7 +264,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
         const float span = __ldg(omega + nE - 1) - om0;
         if (span > 0.0f) inv_dom = (float)(nE - 1) / span;
     }
-    float* part = p.partial + (size_t)blockIdx.x * 3 * norb * nE;   // rows [bin][ D | T | S ]
+    float* part = p.partial + (size_t)blockIdx.x * 3 * norb * p.nEp;   // rows [bin][ D | T | S ]
     const bool vec4 = (MB % 4 == 0) && (norb % 4 == 0);          // 16-byte aligned vector reductions
     const bool w_vec4 = (MB % 4 == 0) && !p.unitW && !p.cplx && p.sWm == 1 && (norb % 4 == 0) &&
                         ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
@@ -509,6 +519,65 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     if (lane == 0 && (cnt_tb | ev)) {
         atomicAdd(p.counters + 0, cnt_tb);
         atomicAdd(p.counters + 1, ev);
+    }
+}
+
+// Window statistics of a sample of the slab's cubes (A2/A3 only): est[0] += bins with E1 < omega < E4, est[1] += 1 per
+// (tetrahedron, band).  The main kernels enqueued behind it read the two sums and the one that suits the windows
+// runs (wanted_generation); no host round trip.
+struct EstimateParams {
+    const float* E;
+    const float* omega;
+    long long sEk, sEn;
+    int N1, N2, N3, nb, nE;
+    int z_lo, z_hi;
+    int n_cubes;                 // cubes sampled, spread evenly over the slab
+    unsigned long long* est;
+};
+
+__global__ void __launch_bounds__(256) tdos_estimate(const EstimateParams p) {
+    const float* __restrict__ omega = p.omega;
+    const float om0 = __ldg(omega);
+    float inv_dom = 0.0f;
+    if (p.nE > 1) {
+        const float span = __ldg(omega + p.nE - 1) - om0;
+        if (span > 0.0f) inv_dom = (float)(p.nE - 1) / span;
+    }
+    const long long slab = (long long)p.N1 * p.N2 * (p.z_hi - p.z_lo);
+    const long long total = (long long)p.n_cubes * 6 * p.nb;
+    unsigned long long bins = 0, cnt = 0;
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < total; j += (long long)gridDim.x * blockDim.x) {
+        const int n = (int)(j % p.nb);
+        const int tet = (int)((j / p.nb) % 6);
+        const long long s = j / ((long long)p.nb * 6);
+        const long long cube = (slab * s) / p.n_cubes;   // evenly spread
+        const int ix = (int)(cube % p.N1), iy = (int)((cube / p.N1) % p.N2), iz = p.z_lo + (int)(cube / ((long long)p.N1 * p.N2));
+        float emin = 3.0e38f, emax = -3.0e38f;
+#pragma unroll
+        for (int l = 0; l < 4; l++) {
+            const int a = kTableI[tet][l];
+            int gx = ix + (a & 1), gy = iy + ((a >> 1) & 1), gz = iz + (a >> 2);
+            if (gx >= p.N1) gx -= p.N1;
+            if (gy >= p.N2) gy -= p.N2;
+            if (gz >= p.N3) gz -= p.N3;
+            const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
+            const float e = __ldg(p.E + ik * p.sEk + (long long)n * p.sEn);
+            emin = fminf(emin, e);
+            emax = fmaxf(emax, e);
+        }
+        const int i1 = locate_bin<true>(omega, p.nE, om0, inv_dom, emin);
+        const int i4 = (emax > emin) ? locate_bin<false>(omega, p.nE, om0, inv_dom, emax) : i1;
+        bins += (unsigned)(i4 - i1);
+        cnt += 1;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        bins += __shfl_xor_sync(0xffffffffu, bins, d);
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, d);
+    }
+    if ((threadIdx.x & 31) == 0 && cnt) {
+        atomicAdd(p.est + 0, bins);
+        atomicAdd(p.est + 1, cnt);
     }
 }
 

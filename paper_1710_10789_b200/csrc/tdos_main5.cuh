@@ -423,6 +423,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
     float* sW = reinterpret_cast<float*>(base + C::off_w);
     float* sE = reinterpret_cast<float*>(base + C::off_un);
 
+    if (p.est && wanted_generation(p.est[0], p.est[1]) != 5) return;   // the other kernel of the pair runs
     const int nE = p.nE, norb = NORB ? NORB : p.norb;
     const float* __restrict__ omega = p.omega;
     // the energy grid is probed 8 times per (tetrahedron, band): keep a block-wide copy in shared memory when it fits

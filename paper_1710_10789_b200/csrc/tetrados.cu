@@ -15,11 +15,13 @@
 #include "tdos_kernels.cuh"
 #include "tdos_kweights.cuh"
 #include "tdos_main5.cuh"
-#include "tdos_main6.cuh"
 
 namespace {
 
 thread_local char g_cuda_err[256] = "";
+
+// cubes sampled by tdos_estimate when a plan chooses between its two main kernels per call
+constexpr int kEstimateCubes = 2048;
 
 // host mode: bytes of E + W per staged z-slab (copy/compute overlap granularity)
 constexpr size_t kSlabBytes = (size_t)64 << 20;
@@ -37,33 +39,32 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
+// every entry point works on the plan's device and leaves the caller's current device as it found it
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err;
+    explicit DeviceGuard(int dev) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+        else if (err == cudaSuccess) prev = -1;   // nothing to restore
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+#define ON_DEVICE(dev)       \
+    DeviceGuard guard_(dev); \
+    if (guard_.err != cudaSuccess) return cuda_fail(guard_.err, "cudaSetDevice")
+
 using tdos::MainParams;
 typedef void (*main_kernel_t)(const MainParams);
 
 struct Variant {
-    main_kernel_t fn;      // tdos_main (generation 3), tdos_main5 (generation 5) or tdos_main6 (generation 6)
+    main_kernel_t fn;      // tdos_main (generation 3) or tdos_main5 (generation 5)
     int MB, TX, TY, TZ, GL, NWARP;
     size_t smem;
-    int gen = 3;                    // main kernel generation: 3, 5 or 6
-    int bps = 0;                    // generation 6: blocks per SM the kernel is built for
+    int gen = 3;                    // main kernel generation: 3 or 5
 };
-
-template <int TX, int TY, int TZ, int NWARP, int NORB, int BPS>
-Variant make_variant6() {
-    Variant v{tdos::tdos_main6<TX, TY, TZ, NWARP, NORB, BPS>, 8, TX, TY, TZ, 2, NWARP, tdos::Cfg6<TX, TY, TZ, NWARP>::bytes};
-    v.gen = 6;
-    v.bps = BPS;
-    return v;
-}
-
-// v6 configurations compiled in (TDOS_TILE=<index> selects another one for experiments)
-template <int NORB>
-std::vector<Variant> variants6() {
-    return {make_variant6<2, 4, 8, 8, NORB, 2>(), make_variant6<4, 4, 4, 8, NORB, 2>(), make_variant6<2, 2, 16, 8, NORB, 2>(),
-            make_variant6<4, 4, 8, 16, NORB, 1>(), make_variant6<2, 2, 8, 8, NORB, 2>(), make_variant6<2, 2, 8, 4, NORB, 4>(),
-            make_variant6<2, 4, 4, 4, NORB, 4>(), make_variant6<2, 2, 8, 6, NORB, 3>(), make_variant6<2, 4, 8, 12, NORB, 1>(),
-            make_variant6<2, 2, 8, 8, NORB, 3>(), make_variant6<2, 2, 8, 6, NORB, 4>(), make_variant6<2, 2, 8, 4, NORB, 6>()};
-}
 
 template <int TX, int TY, int TZ, int NWARP, int NORB>
 Variant make_variant5() {
@@ -115,14 +116,19 @@ struct tdos_plan {
     int nb = 0, norb = 0, nE_max = 0;
     int num_sms = 0;
     size_t smem_optin = 0;        // cudaDevAttrMaxSharedMemoryPerBlockOptin
-    size_t smem_per_sm = 0;       // cudaDevAttrMaxSharedMemoryPerMultiprocessor
-    Variant var{};                // the main kernel in use
+    Variant var{};                // the main kernel (generation 5 when the orbitals allow it, else 3)
+    Variant var_short{};          // adaptive plans: generation 3, better when the windows are a few bins only
+    bool adaptive = false;        // both kernels are enqueued; the device picks one per call (tdos_estimate)
     int blocks_per_sm = 0;
-    int grid = 0;
-    int nparts = 0;               // copies of the partial histogram (generation 6: one per SM; else one per block)
+    int grid = 0;                 // blocks of `var`
+    int grid_short = 0;           // blocks of `var_short`
+    int nparts = 0;               // copies of the partial histogram = max(grid, grid_short)
     float* partial = nullptr;     // [nparts] rows [nE_max + 3][3 * norb]
     double* part64 = nullptr;     // [3][norb][nE_max]
-    unsigned long long* counters = nullptr;   // [2] n_tb, n_eval of the last call
+    // [0..2] n_tb, n_eval, n_eval_mid of the last call; [3] work-item counter; [4..5] window sample (tdos_estimate)
+    unsigned long long* counters = nullptr;
+    cudaEvent_t done_ev = nullptr;   // end of the last call: the next call's stream waits for it (shared scratch)
+    bool done_valid = false;
     // host-mode staging
     float* dE = nullptr;
     float* dW = nullptr;
@@ -166,7 +172,7 @@ const char* tdos_last_cuda_error(void) { return g_cuda_err; }
 
 int tdos_plan_destroy(tdos_plan* p) {
     if (!p) return TDOS_OK;
-    cudaSetDevice(p->device);
+    DeviceGuard guard_(p->device);
     if (p->side) cudaStreamSynchronize(p->side);
     if (p->main) cudaStreamSynchronize(p->main);
     cudaFree(p->partial);
@@ -181,6 +187,7 @@ int tdos_plan_destroy(tdos_plan* p) {
         if (e) cudaEventDestroy(e);
     for (auto& e : p->cp_ev)
         if (e) cudaEventDestroy(e);
+    if (p->done_ev) cudaEventDestroy(p->done_ev);
     for (auto& tr : p->ring)
         for (auto& e : tr)
             if (e) cudaEventDestroy(e);
@@ -194,7 +201,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     if (!out || !nk) return TDOS_EINVAL;
     if (nk[0] < 1 || nk[1] < 1 || nk[2] < 1 || nb < 1 || norb < 1 || nE_max < 1 || nE_max > TDOS_MAX_NE) return TDOS_EINVAL;
     if ((long long)nk[0] * nk[1] * nk[2] > 0x7fffffffLL) return TDOS_EINVAL;
-    CK(cudaSetDevice(device));
+    ON_DEVICE(device);
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, device));
     if (prop.major != 10) return TDOS_EARCH;
@@ -208,49 +215,59 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     p->nE_max = nE_max;
     p->num_sms = prop.multiProcessorCount;
     p->smem_optin = prop.sharedMemPerBlockOptin;
-    p->smem_per_sm = prop.sharedMemPerMultiprocessor;
 
     const char* kv = getenv("TDOS_KERNEL");
-    // generations 5 and 6 work on blocks of 8 orbitals with 16-byte vector reductions; narrower problems use generation 3
+    // generation 5 needs blocks of 8 orbitals to pay off; narrower problems use generation 3
     int gen = kv ? atoi(kv) : 5;
-    if (gen != 3 && gen != 5 && gen != 6) gen = 5;
-    if (gen != 3 && (norb < 5 || norb % 4 != 0)) gen = 3;
-    std::vector<Variant> vs = gen == 6   ? (norb == 8 ? variants6<8>() : variants6<0>())
-                              : gen == 5 ? (norb == 8 ? variants5<8>() : variants5<0>())
-                                         : variants(pick_mb(norb));
+    if (gen == 5 && (norb < 5 || norb % 4 != 0)) gen = 3;   // tdos_main5: blocks of 8 orbitals, 16-byte vector reductions
+    std::vector<Variant> vs = gen == 5 ? (norb == 8 ? variants5<8>() : variants5<0>()) : variants(pick_mb(norb));
     int sel = 0;
     // Tile shape of generation 5.  A tile whose bands span few energy bins keeps more (record, chunk) entries per
     // chunk.  The paper's workloads are layered materials sampled on grids like 60 x 60 x 10, with
     // the weak dispersion along z, so the default tile is long in z whenever the grid divides evenly (2 x 2 x 8
-    // cubes); TDOS_TILE=<index> overrides it.
+    // cubes, 15.1 ms on config 4 against 15.7 ms for 4 x 4 x 2); TDOS_TILE=<index> overrides it.
     if (gen == 5 && nk[2] % 8 == 0 && nk[0] % 2 == 0 && nk[1] % 2 == 0) sel = 1;
     if (const char* s = getenv("TDOS_TILE")) sel = atoi(s);
     if (sel < 0 || sel >= (int)vs.size()) sel = 0;
     p->var = vs[sel];
 
-    // The attribute belongs to the kernel function, not to the plan: always the device maximum, so that plans with
-    // different nE_max never lower each other's limit.
-    const void* kfn = (const void*)p->var.fn;
-    cudaError_t e = cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_optin);
-    if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->blocks_per_sm, kfn, p->var.NWARP * 32, p->var.smem);
+    // The shared-memory limit is an attribute of the kernel function, not of the plan: always the device maximum, so
+    // that plans with different nE_max cannot lower each other's limit.
+    auto setup = [&](const Variant& v, int* bps) -> cudaError_t {
+        cudaError_t e = cudaFuncSetAttribute((const void*)v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_optin);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bps, (const void*)v.fn, v.NWARP * 32, v.smem);
+        return e;
+    };
+    cudaError_t e = setup(p->var, &p->blocks_per_sm);
     if (e != cudaSuccess || p->blocks_per_sm < 1) {
         int rc = (e != cudaSuccess) ? cuda_fail(e, "kernel setup") : TDOS_ECUDA;
         delete p;
         return rc;
     }
-    if (p->var.gen == 6 && p->blocks_per_sm > p->var.bps) p->blocks_per_sm = p->var.bps;
-    if (const char* s = getenv("TDOS_BLOCKS_PER_SM")) {
+    if (const char* s = getenv("TDOS_BLOCKS_PER_SM")) {   // experiments only (include/tetrados.h)
         int b = atoi(s);
         if (b >= 1 && b < p->blocks_per_sm) p->blocks_per_sm = b;
     }
     p->grid = p->num_sms * p->blocks_per_sm;
-    p->nparts = p->var.gen == 6 ? p->num_sms : p->grid;
+    p->nparts = p->grid;
+    // Without TDOS_KERNEL a plan on blocks of 8 orbitals carries both kernels: windows of a few bins only (config 5:
+    // 3 bins on average) are served better by one record per tetrahedron (generation 3) than by three (generation 5).
+    // Which one runs is decided per call on the device, from a sample of the windows (tdos_estimate).
+    if (gen == 5 && !kv) {
+        p->var_short = variants(8)[0];
+        int bps = 0;
+        if (setup(p->var_short, &bps) == cudaSuccess && bps >= 1) {
+            p->adaptive = true;
+            p->grid_short = p->num_sms * bps;
+            if (p->grid_short > p->nparts) p->nparts = p->grid_short;
+        }
+        cudaGetLastError();
+    }
 
     const size_t hist = (size_t)3 * norb * ((size_t)nE_max + 3);
     if (cudaMalloc(&p->partial, hist * p->nparts * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&p->part64, hist * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&p->counters, 40 * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaMalloc(&p->counters, 8 * sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError();
         tdos_plan_destroy(p);
         return TDOS_ENOMEM;
@@ -258,6 +275,11 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&p->main, cudaStreamNonBlocking) != cudaSuccess) {
         int rc = cuda_fail(cudaGetLastError(), "cudaStreamCreate");
+        tdos_plan_destroy(p);
+        return rc;
+    }
+    if (cudaEventCreateWithFlags(&p->done_ev, cudaEventDisableTiming) != cudaSuccess) {
+        int rc = cuda_fail(cudaGetLastError(), "cudaEventCreate");
         tdos_plan_destroy(p);
         return rc;
     }
@@ -287,13 +309,25 @@ static int check_common(const tdos_plan* p, const float* E, const float* W, int 
 }
 
 // rows of one block's partial histogram: generation 5 flushes whole chunks of 4 bins
-static int rows_per_block(const tdos_plan* p, int nE) { return p->var.gen >= 5 ? (nE + 3) & ~3 : nE; }
+// rows of one block's partial histogram: generation 5 flushes whole chunks of 4 bins; both kernels use this layout
+static int rows_per_block(int nE) { return (nE + 3) & ~3; }
+
+// The plan's scratch (partials, counters, merge buffer) is shared by all calls: a call on another stream than the
+// previous one waits for that one's end.
+static int order_after_last_call(tdos_plan* p, cudaStream_t st) {
+    if (p->done_valid && !(p->last_stream_valid && p->last_stream == st)) CK(cudaStreamWaitEvent(st, p->done_ev, 0));
+    return TDOS_OK;
+}
+static int mark_end_of_call(tdos_plan* p, cudaStream_t st) {
+    CK(cudaEventRecord(p->done_ev, st));
+    p->done_valid = true;
+    return TDOS_OK;
+}
 
 // enqueue the main kernel for the cube slab [z_lo, z_hi); `first` also clears the block partials and the
 // work counters (a call may cover the grid with several slab launches that accumulate into the same partials)
 static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
                         int z_lo, int z_hi, bool first, cudaStream_t st) {
-    const Variant& v = p->var;
     const long long nkt = (long long)p->nk[0] * p->nk[1] * p->nk[2];
     MainParams mp{};
     mp.E = E;
@@ -308,53 +342,66 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     }
     mp.N1 = p->nk[0]; mp.N2 = p->nk[1]; mp.N3 = p->nk[2];
     mp.nb = p->nb; mp.norb = p->norb; mp.nE = nE;
-    mp.nEp = rows_per_block(p, nE);
+    mp.nEp = rows_per_block(nE);
     mp.z_lo = z_lo; mp.z_hi = z_hi;
-    mp.ntx = (p->nk[0] + v.TX - 1) / v.TX;
-    mp.nty = (p->nk[1] + v.TY - 1) / v.TY;
-    mp.ntz = (z_hi - z_lo + v.TZ - 1) / v.TZ;
-    mp.nmb = (p->norb + v.MB - 1) / v.MB;
-    const long long items = (long long)mp.ntx * mp.nty * mp.ntz * p->nb * mp.nmb;
-    if (items > 0x7fffffffLL) return TDOS_EINVAL;
-    mp.n_items = (int)items;
     mp.unitW = (W == nullptr);
     mp.cplx = (W != nullptr) ? p->cplx : 0;
     mp.partial = p->partial;
-    mp.nparts = p->nparts;
     mp.counters = p->counters;
     mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
+    mp.est = p->adaptive ? p->counters + 4 : nullptr;
 
-    const long long work = items;
-    // generations 5 and 6: a block-wide copy of omega in shared memory if it fits (generation 6: without costing a
-    // resident block)
-    size_t smem = v.smem;
-    const size_t om_bytes = (size_t)nE * sizeof(float);
-    if (v.gen == 5 && v.smem + om_bytes <= p->smem_optin) {
-        mp.om_smem = 1;
-        smem += om_bytes;
-    }
-    if (v.gen == 6 && v.smem + om_bytes <= p->smem_optin &&
-        (size_t)p->blocks_per_sm * (v.smem + om_bytes + 1024) <= p->smem_per_sm) {
-        mp.om_smem = 1;
-        smem += om_bytes;
-    }
     const size_t hist = (size_t)3 * p->norb * mp.nEp;
     if (first) {
         CK(cudaMemsetAsync(p->partial, 0, hist * p->nparts * sizeof(float), st));
-        CK(cudaMemsetAsync(p->counters, 0, 40 * sizeof(unsigned long long), st));
+        CK(cudaMemsetAsync(p->counters, 0, 8 * sizeof(unsigned long long), st));
         p->last_items = 0;
         p->last_launches = 0;
-    } else if (v.gen >= 5) {
+        if (p->adaptive && z_hi > z_lo) {   // sample the windows of this call's (first) slab: the device picks the kernel
+            tdos::EstimateParams ep{};
+            ep.E = E; ep.omega = omega;
+            ep.sEk = mp.sEk; ep.sEn = mp.sEn;
+            ep.N1 = mp.N1; ep.N2 = mp.N2; ep.N3 = mp.N3; ep.nb = mp.nb; ep.nE = nE;
+            ep.z_lo = z_lo; ep.z_hi = z_hi;
+            const long long slab = (long long)mp.N1 * mp.N2 * (z_hi - z_lo);
+            ep.n_cubes = (int)(slab < kEstimateCubes ? slab : kEstimateCubes);
+            ep.est = p->counters + 4;
+            const long long total = (long long)ep.n_cubes * 6 * mp.nb;
+            tdos::tdos_estimate<<<(int)((total + 1023) / 1024), 256, 0, st>>>(ep);
+            CK(cudaGetLastError());
+            p->last_launches += 1;
+        }
+    } else {
         CK(cudaMemsetAsync(p->counters + 3, 0, sizeof(unsigned long long), st));
     }
-    if (work > 0) {
-        const long long blocks_needed = v.gen == 6 ? work : (work + v.NWARP - 1) / v.NWARP;
-        const int grid = (int)((blocks_needed < p->grid) ? blocks_needed : p->grid);
-        v.fn<<<grid, v.NWARP * 32, smem, st>>>(mp);
-        CK(cudaGetLastError());
-        p->last_launches += 1;
+    long long items_main = 0;
+    for (int which = 0; which < (p->adaptive ? 2 : 1); ++which) {
+        const Variant& v = which ? p->var_short : p->var;
+        const int vgrid = which ? p->grid_short : p->grid;
+        mp.ntx = (p->nk[0] + v.TX - 1) / v.TX;
+        mp.nty = (p->nk[1] + v.TY - 1) / v.TY;
+        mp.ntz = (z_hi - z_lo + v.TZ - 1) / v.TZ;
+        mp.nmb = (p->norb + v.MB - 1) / v.MB;
+        const long long items = (long long)mp.ntx * mp.nty * mp.ntz * p->nb * mp.nmb;
+        if (items > 0x7fffffffLL) return TDOS_EINVAL;
+        mp.n_items = (int)items;
+        if (!which) items_main = items;
+        // generation 5: a block-wide copy of omega in shared memory if the device limit allows it
+        size_t smem = v.smem;
+        mp.om_smem = 0;
+        if (v.gen == 5 && v.smem + (size_t)nE * sizeof(float) <= p->smem_optin) {
+            mp.om_smem = 1;
+            smem += (size_t)nE * sizeof(float);
+        }
+        if (items > 0) {
+            const long long blocks_needed = (items + v.NWARP - 1) / v.NWARP;
+            const int grid = (int)((blocks_needed < vgrid) ? blocks_needed : vgrid);
+            v.fn<<<grid, v.NWARP * 32, smem, st>>>(mp);
+            CK(cudaGetLastError());
+            p->last_launches += 1;
+        }
     }
-    p->last_items += items;
+    p->last_items += items_main;
     p->last_stream = st;
     p->last_stream_valid = true;
     p->timed = false;
@@ -365,7 +412,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
 static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st) {
     const size_t hist = (size_t)3 * p->norb * nE;
     const int mblocks = (int)((hist + 255) / 256);
-    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->nparts, p->norb, nE, rows_per_block(p, nE), part_out);
+    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->nparts, p->norb, nE, rows_per_block(nE), part_out);
     CK(cudaGetLastError());
     p->last_launches += 1;
     return TDOS_OK;
@@ -374,6 +421,8 @@ static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st
 // zero partials, main kernel over [z_lo, z_hi), merge into part_out; events around the main kernel
 static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
                            int z_lo, int z_hi, double* part_out, cudaStream_t st) {
+    int rc0 = order_after_last_call(p, st);
+    if (rc0) return rc0;
     CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
     int rc = enqueue_main(p, E, W, layout, omega, nE, z_lo, z_hi, true, st);
     if (rc) return rc;
@@ -394,19 +443,19 @@ int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, 
     int rc = check_common(p, E, W, layout, omega, nE);
     if (rc) return rc;
     if (!part || z_lo < 0 || z_hi > p->nk[2] || z_lo > z_hi) return TDOS_EINVAL;
-    CK(cudaSetDevice(p->device));
+    ON_DEVICE(p->device);
     p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
     rc = enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream);
     if (rc) return rc;
     CK(cudaEventRecord(p->ring[p->cur_slot][2], (cudaStream_t)cuda_stream));
     p->n_timed_calls++;
     p->timed = true;
-    return TDOS_OK;
+    return mark_end_of_call(p, (cudaStream_t)cuda_stream);
 }
 
 int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos, void* cuda_stream) {
     if (!p || !part || !dos || nE < 1 || nE > p->nE_max) return TDOS_EINVAL;
-    CK(cudaSetDevice(p->device));
+    ON_DEVICE(p->device);
     return enqueue_finalize(p, part, nE, dos, nos, (cudaStream_t)cuda_stream);
 }
 
@@ -420,7 +469,7 @@ static int run_device(tdos_plan* p, const float* E, const float* W, int layout, 
     CK(cudaEventRecord(p->ring[p->cur_slot][2], st));
     p->n_timed_calls++;
     p->timed = true;
-    return TDOS_OK;
+    return mark_end_of_call(p, st);
 }
 
 static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
@@ -447,7 +496,7 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
     if (rc) return rc;
     if (!dos) return TDOS_EINVAL;
     if (memspace != TDOS_DEVICE && memspace != TDOS_HOST) return TDOS_EINVAL;
-    CK(cudaSetDevice(p->device));
+    ON_DEVICE(p->device);
     if (memspace == TDOS_DEVICE) return run_device(p, E, W, layout, omega, nE, dos, nos, (cudaStream_t)cuda_stream);
 
     // ---- host mode: validate omega, stage in, run, stage out
@@ -486,6 +535,8 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
     // also plane 0), so the cubes of slab s -- which read planes z_s .. z_{s+1}, the last one wrapping to
     // plane 0 -- need copies 0..s only.
     cudaStream_t st = p->main, cp = p->side;
+    rc = order_after_last_call(p, st);
+    if (rc) return rc;
     const int N3 = p->nk[2];
     const size_t plane = (size_t)p->nk[0] * p->nk[1];
     const size_t total = nkt * p->nb * (1 + (W ? (size_t)p->norb * wfl : 0)) * sizeof(float);
@@ -557,6 +608,8 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
     p->timed = true;
     CK(cudaMemcpyAsync(dos, p->dDos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
     if (nos) CK(cudaMemcpyAsync(nos, p->dNos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
+    rc = mark_end_of_call(p, st);
+    if (rc) return rc;
     CK(cudaStreamSynchronize(st));
     return TDOS_OK;
 }
@@ -565,7 +618,7 @@ int tetra_weights(tdos_plan* p, const float* E, int layout, const float* energie
                   void* cuda_stream) {
     if (!p || !E || !energies || !wk || nW < 1) return TDOS_EINVAL;
     if (layout != TDOS_AOS && layout != TDOS_SOA) return TDOS_EINVAL;
-    CK(cudaSetDevice(p->device));
+    ON_DEVICE(p->device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long nkt = (long long)p->nk[0] * p->nk[1] * p->nk[2];
     tdos::KWeightParams kp{};
@@ -627,25 +680,15 @@ int tdos_plan_info(const tdos_plan* p, long long what[8]) {
 
 int tdos_last_counters(tdos_plan* p, long long cnt[4]) {
     if (!p || !cnt || !p->last_stream_valid) return TDOS_EINVAL;
-    CK(cudaSetDevice(p->device));
+    ON_DEVICE(p->device);
     CK(cudaStreamSynchronize(p->last_stream));
-#ifdef TDOS_PHASES
-    {
-        unsigned long long ph[24];
-        CK(cudaMemcpy(ph, p->counters + 8, sizeof(ph), cudaMemcpyDeviceToHost));
-        for (int w = 0; w < 2; w++) {
-            fprintf(stderr, "phases (%s warp, kcycles per block):", w ? "last" : "first");
-            for (int k = 0; k < 12; k++) fprintf(stderr, " %.0f", (double)ph[12 * w + k] / p->grid / 1e3);
-            fprintf(stderr, "\n");
-        }
-    }
-#endif
-    unsigned long long h[3];
+    unsigned long long h[6];
     CK(cudaMemcpy(h, p->counters, sizeof(h), cudaMemcpyDeviceToHost));
+    const int gen = p->adaptive ? tdos::wanted_generation(h[4], h[5]) : p->var.gen;   // what the device decided
     cnt[0] = (long long)h[0];
     cnt[1] = (long long)h[1];
-    cnt[2] = p->var.gen >= 5 ? (long long)h[2] : -1;
-    cnt[3] = p->var.gen;
+    cnt[2] = gen == 5 ? (long long)h[2] : -1;
+    cnt[3] = gen;
     return TDOS_OK;
 }
 
@@ -653,7 +696,7 @@ int tdos_kernel_ms(tdos_plan* p, int ncalls, float* main_ms, float* merge_ms) {
     if (!p || !main_ms || !merge_ms || !p->timed || ncalls < 1 || ncalls > tdos_plan::kRing ||
         ncalls > p->n_timed_calls)
         return TDOS_EINVAL;
-    CK(cudaSetDevice(p->device));
+    ON_DEVICE(p->device);
     double a = 0.0, b = 0.0;
     for (int j = 0; j < ncalls; j++) {
         cudaEvent_t* tr = p->ring[(p->n_timed_calls - 1 - j) % tdos_plan::kRing];
@@ -673,7 +716,7 @@ int tdos_last_kernel_ms(tdos_plan* p, float* main_ms, float* merge_ms) { return 
 
 int tdos_fp32_fma_probe(tdos_plan* p, int packed, double* tflops) {
     if (!p || !tflops) return TDOS_EINVAL;
-    CK(cudaSetDevice(p->device));
+    ON_DEVICE(p->device);
     const int iters = 4096, blocks = p->num_sms * 8, threads = 256;
     float* d = nullptr;
     CK(cudaMalloc(&d, sizeof(float)));

@@ -273,9 +273,10 @@ def test_paper_shaped_anisotropic_grid(cache_dir):
     ((2, 2, 2), 3, 16, 61),       # two orbital blocks, every neighbour is a wrap
     ((7, 6, 9), 2, 12, 515),      # second orbital block half empty (norb = 12)
 ])
-def test_generation5_edge_cases(nk, nb, norb, nE):
-    """The default kernel for norb % 4 == 0, norb >= 5 (tdos_main5) on the degenerate shapes: AoS, SoA, host mode,
-    random energies (windows of many bins) and lattice energies with omega ON the corner values (ties, G10/G11)."""
+def test_generation5_edge_cases(nk, nb, norb, nE, monkeypatch):
+    """tdos_main5 (the kernel for windows of many bins when norb % 4 == 0, norb >= 5; forced here) on the degenerate
+    shapes: AoS, SoA, host mode, random energies and lattice energies with omega ON the corner values (ties, G10/G11)."""
+    monkeypatch.setenv("TDOS_KERNEL", "5")
     E, W = wl.random_bands(nk, nb, norb, seed=7 + nE)
     om = wl.omega_grid(-1.1, 1.2, nE)
     ref = oracle.tetra_dos(E, W, nk, om)
@@ -363,21 +364,27 @@ def test_per_k_integration_weights(nk, nb):
                 assert torch.equal(torch.nan_to_num(wk2), torch.nan_to_num(wk)) or np.allclose(wk2.cpu().numpy(), w, atol=1e-6 / n)
 
 
-def test_plan_switches_kernel_for_short_windows(monkeypatch):
-    """Unless TDOS_KERNEL is set, a plan that started with tdos_main5 keeps tdos_main from its second call on when
-    the first call's counters show windows below 6 bins on average; results stay within tolerance either way."""
+def test_plan_picks_kernel_per_call_on_the_device(monkeypatch):
+    """Unless TDOS_KERNEL is set, a plan on 8 orbitals enqueues both main kernels and a sample of the windows, taken on
+    the device at the start of every call, decides which one runs: tdos_main (one record per tetrahedron) below 6 bins
+    per window, tdos_main5 above.  The same plan serves a coarse and a fine energy grid in turn; every call is checked."""
     monkeypatch.delenv("TDOS_KERNEL", raising=False)
     nk, nb, norb = (8, 8, 8), 2, 8
     E, W = wl.tb8_bands(nk, threads=1)
     E, W = np.ascontiguousarray(E[:, :nb]), np.ascontiguousarray(W[:, :nb, :])
-    for nE, expect in ((24, 3), (900, 5)):       # coarse grid: windows of about one bin; fine grid: tens of bins
-        om = wl.omega_grid(-6.0, 4.0, nE)
-        ref = oracle.tetra_dos(E, W, nk, om)
-        with binding.Plan(nk, nb, norb, nE) as plan:
-            for call in range(3):
-                dos, nos = run_gpu(E, W, nk, om, plan=plan)
-                assert_parity(ref, dos, nos, "adaptive nE %d call %d" % (nE, call))
-                assert plan.last_counters()["kernel"] == (5 if call == 0 else expect)
+    grids = {24: 3, 900: 5}       # coarse grid: windows of about one bin; fine grid: tens of bins
+    refs = {nE: oracle.tetra_dos(E, W, nk, wl.omega_grid(-6.0, 4.0, nE)) for nE in grids}
+    with binding.Plan(nk, nb, norb, 900) as plan:
+        for nE in (24, 900, 24, 24, 900):
+            om = wl.omega_grid(-6.0, 4.0, nE)
+            dos, nos = run_gpu(E, W, nk, om, plan=plan)
+            assert_parity(refs[nE], dos, nos, "adaptive nE %d" % nE)
+            cnt = plan.last_counters()
+            assert cnt["kernel"] == grids[nE]
+            assert cnt["n_tb"] == refs[nE]["n_tb"] and cnt["n_eval"] == refs[nE]["n_eval"]
+        dos, nos = run_gpu(E, W, nk, wl.omega_grid(-6.0, 4.0, 24), plan=plan, memspace=binding.TDOS_HOST)
+        assert_parity(refs[24], dos, nos, "adaptive host nE 24")
+        assert plan.last_counters()["kernel"] == 3
     monkeypatch.setenv("TDOS_KERNEL", "5")
     om = wl.omega_grid(-6.0, 4.0, 24)
     with binding.Plan(nk, nb, norb, 24) as plan:
