@@ -190,8 +190,9 @@ def workload_config(cfg, n_gpus: int) -> dict:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the main kernel, from the committed
 # `ncu --set full` capture (profiles/, named there); None until a capture of that config exists.
-NCU_TRAFFIC_BYTES = {("cfg4", 3): 1.394956e9 + 280.968e6,    # profiles/r01_v3_regions_cfg4.md
-                     ("cfg4", 5): 731.369e6 + 80.145e6}    # profiles/r01_v5_main_cfg4.md
+# The number is a constant from that file, NOT measured in this run: `roofline.traffic_source` names the file.
+NCU_TRAFFIC_BYTES = {("cfg4", 3): (1.394956e9 + 280.968e6, "profiles/r01_v3_regions_cfg4.md"),
+                     ("cfg4", 5): (731.369e6 + 80.145e6, "profiles/r01_v5_main_cfg4.md")}
 
 
 def main():
@@ -206,7 +207,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1710_10789_b200 import binding, sharding   # raises if libtetrados.so is missing: no CPU fallback
+    from paper_1710_10789_b200 import binding, multigpu, sharding   # raises if libtetrados.so is missing: no CPU fallback
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
@@ -240,10 +241,8 @@ def main():
     def step():
         if world == 1:
             plan.tetra_dos(dE, dW, dOm, dos, nos)
-        else:
-            plan.tetra_dos_partial(dE, dW, dOm, z_lo, z_hi, part)
-            dist.all_reduce(part)                      # the path's one exchange step
-            plan.tetra_dos_finalize(part, nE, dos, nos)
+        else:   # partial over this rank's z-slab -> ONE all-reduce (the path's only exchange step) -> finalize
+            multigpu.sharded_step(plan, dE, dW, dOm, N3, rank, world, part, dos, nos, dist.all_reduce)
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -277,7 +276,9 @@ def main():
         main_ms = float(km.item())
     n_tb, n_eval, n_mid = int(c[0].item()), int(c[1].item()), int(c[2].item())
     info = plan.info()
-    launches_per_step = 3   # main + merge + finalize (memsets and NCCL not counted)
+    # kernels of this library launched per step, counted by the library itself (adaptive plans: window sample + both
+    # main kernels, one of which returns at once; then merge and finalize; memsets and NCCL not counted)
+    launches_per_step = int(info["launches"])
 
     # ---- e2e: the same step through the C-ABI with HOST (pinned) buffers
     e2e = None
@@ -324,21 +325,46 @@ def main():
         h2d = E.nbytes + (0 if unitW else W.nbytes) + om.nbytes
         if world > 1:   # halo planes are copied twice across the job
             h2d += world * plane * 4 * nb * (1 + (0 if unitW else norb)) + (world - 1) * om.nbytes
+        # reference for the achieved host->device rate: ONE plain
+        # cudaMemcpyAsync of the same E + W bytes from the same pinned buffers, nothing overlapped with it
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        plain = []
+        for _ in range(3):
+            torch.cuda.synchronize()
+            c0.record()
+            dE.copy_(hE, non_blocking=True)
+            if hW is not None:
+                dW.copy_(hW, non_blocking=True)
+            c1.record()
+            torch.cuda.synchronize()
+            plain.append(c0.elapsed_time(c1) * 1e-3)
+        copy_bytes = E.nbytes + (0 if unitW else W.nbytes)
         e2e = {"value": n_tb * nE / e2e_s, "unit": "eval/s", "ms_per_step": e2e_s * 1e3,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(2 * norb * nE * 4),
-               "h2d_gbs": h2d / e2e_s / 1e9}
+               "h2d_gbs": h2d / e2e_s / 1e9,
+               "h2d_gbs_plain": copy_bytes / min(plain) / 1e9, "plain_copy_ms": min(plain) * 1e3,
+               "note": "h2d_gbs = staged bytes / whole e2e step (copies overlapped with the kernels); h2d_gbs_plain = one "
+                       "plain cudaMemcpyAsync of the same E + W bytes from the same pinned buffers, timed alone"}
 
     # ---- roofline of the dominant kernel (tdos_main): FP32 ALU
     props = torch.cuda.get_device_properties(dev)
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak = fp32_peak_tflops(props.multi_processor_count, sm_max)
+    # `achieved` / `frac`: SURVEY.md 8(d)'s per-unit counts (the method as the paper states it) x the units the kernel
+    # itself counted -- the count the north star's 60 % target is read against.  The kernel's own
+    # formulation needs fewer flops (H, J hoisted for Eq. 12/14); that recount is reported beside it.
     fl_paper = flops_alg(n_eval, n_tb, norb) / world    # per launch (each rank's share on average)
-    fl = flops_alg_gen5(n_eval, n_mid, n_tb, norb) / world if gen == 5 else fl_paper
+    fl_kernel = flops_alg_gen5(n_eval, n_mid, n_tb, norb) / world if gen == 5 else fl_paper
+    fl = fl_paper
     achieved = fl / (main_ms * 1e-3) / 1e12
     bytes_alg = 4.0 * N1 * N2 * N3 * nb * (1 + (0 if unitW else norb)) + 8.0 * norb * nE
+    traffic = NCU_TRAFFIC_BYTES.get((cfg.name, gen))
     roofline = {"bound": "alu", "kernel": "tdos_main5" if gen == 5 else "tdos_main", "achieved": achieved, "peak": peak,
-                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, gen)),
-                "flop_model": "generation-5 formulation (H, J hoisted for Eq. 12/14)" if gen == 5 else "paper formulation",
+                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic[0] if traffic else None,
+                "traffic_source": (traffic[1] + " (constant from that ncu capture, not measured in this run)") if traffic else None,
+                "flop_model": "SURVEY.md 8(d): F_eval = 40 + 18 norb, F_tb = 40 + 5 norb, units counted by the kernel",
+                "frac_kernel_formulation": fl_kernel / (main_ms * 1e-3) / 1e12 / peak,
+                "flops_kernel_formulation_per_launch": fl_kernel,
                 "frac_paper_formulation": fl_paper / (main_ms * 1e-3) / 1e12 / peak,
                 "flops_paper_formulation_per_launch": fl_paper,
                 "peak_source": "derived: %d SMs x 128 FP32 lanes x 2 x %.0f MHz (B200_PROFILING.md unit counts and clocks)"

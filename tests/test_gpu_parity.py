@@ -201,34 +201,63 @@ def test_tetra_dos_simple_host_oneshot():
 # (pinned against the literal one by test_P9_invariances_and_variants) computes every output here,
 # so the comparison is element by element, not sampled; the kernel's exact work counters must equal
 # the oracle's, and the sum rule N_m(omega_max) = (1/nk) sum_k sum_n W (P6) must hold at full size.
-def _full_config(name, cache_dir, host=False):
+_REF_CACHE = {}
+
+
+def _full_ref(name, cache_dir):
+    """inputs and oracle result of a config, computed once per test session"""
+    if name not in _REF_CACHE:
+        cfg = wl.CONFIGS[name]
+        E, W, om = wl.make_inputs(cfg, cache_dir)
+        _REF_CACHE[name] = (E, W, om, oracle.tetra_dos(E, W, cfg.nk, om, windowed=True, nthreads=_threads()))
+    return _REF_CACHE[name]
+
+
+def _full_config(name, cache_dir, host=False, calls=3, expect_kernel=None):
+    """`calls` calls on ONE plan, parity after each: the kernel a plan uses is picked per call on the device, so every
+    call of the sequence is a result a user can get."""
     import torch
     cfg = wl.CONFIGS[name]
-    E, W, om = wl.make_inputs(cfg, cache_dir)
-    ref = oracle.tetra_dos(E, W, cfg.nk, om, windowed=True, nthreads=_threads())
-    with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
-        dos, nos = run_gpu(E, W, cfg.nk, om, plan=plan,
-                           memspace=binding.TDOS_HOST if host else binding.TDOS_DEVICE)
-        cnt = plan.last_counters()
-    d, en = assert_parity(ref, dos, nos, name)
-    assert cnt["n_tb"] == ref["n_tb"] == 6 * int(np.prod(cfg.nk)) * cfg.nb
-    assert cnt["n_eval"] == ref["n_eval"]
+    E, W, om, ref = _full_ref(name, cache_dir)
     total = W.astype(np.float64).sum(axis=(0, 1)) / np.prod(cfg.nk)
-    assert np.allclose(nos[:, -1], total, rtol=2e-6)
-    print("%s%s dDOS %.2e dN %.2e n_eval %d" % (name, " (host)" if host else "", d, en, cnt["n_eval"]))
+    with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
+        for call in range(calls):
+            dos, nos = run_gpu(E, W, cfg.nk, om, plan=plan,
+                               memspace=binding.TDOS_HOST if host else binding.TDOS_DEVICE)
+            cnt = plan.last_counters()
+            d, en = assert_parity(ref, dos, nos, "%s call %d" % (name, call))
+            assert cnt["n_tb"] == ref["n_tb"] == 6 * int(np.prod(cfg.nk)) * cfg.nb
+            assert cnt["n_eval"] == ref["n_eval"]
+            if expect_kernel is not None:
+                assert cnt["kernel"] == expect_kernel
+            assert np.allclose(nos[:, -1], total, rtol=2e-6)
+            print("%s%s call %d kernel %d dDOS %.2e dN %.2e n_eval %d" %
+                  (name, " (host)" if host else "", call, cnt["kernel"], d, en, cnt["n_eval"]))
     torch.cuda.empty_cache()
 
 
 def test_cfg3_full_size(cache_dir):
-    _full_config("cfg3", cache_dir)
+    _full_config("cfg3", cache_dir, expect_kernel=5)
 
 
 def test_cfg4_full_size_headline(cache_dir):
-    _full_config("cfg4", cache_dir)
+    _full_config("cfg4", cache_dir, expect_kernel=5)
 
 
 def test_cfg5_full_size_host_inputs(cache_dir):
-    _full_config("cfg5", cache_dir, host=True)
+    """windows of 3 bins: the device picks tdos_main (generation 3) on every call"""
+    _full_config("cfg5", cache_dir, host=True, calls=2, expect_kernel=3)
+
+
+def test_cfg5_full_size_device_resident(cache_dir):
+    _full_config("cfg5", cache_dir, calls=2, expect_kernel=3)
+
+
+@pytest.mark.parametrize("name,kernel", [("cfg4", 3), ("cfg5", 5)])
+def test_full_size_with_the_other_kernel(name, kernel, cache_dir, monkeypatch):
+    """the kernel the device would not pick for this config, forced: same tolerances at full size"""
+    monkeypatch.setenv("TDOS_KERNEL", str(kernel))
+    _full_config(name, cache_dir, calls=1, expect_kernel=kernel)
 
 
 def test_kernel_generation_3_on_eight_orbitals(monkeypatch):
@@ -391,3 +420,41 @@ def test_plan_picks_kernel_per_call_on_the_device(monkeypatch):
         for call in range(2):
             run_gpu(E, W, nk, om, plan=plan)
             assert plan.last_counters()["kernel"] == 5
+
+
+def test_plans_do_not_lower_each_others_shared_memory_limit():
+    """The dynamic shared-memory limit is an attribute of the kernel function: a second plan with a small nE_max,
+    created (and destroyed) after a plan with a large one, must not break the first."""
+    nk, nb, norb = (8, 8, 8), 2, 8
+    E, W = wl.tb8_bands(nk, threads=1)
+    E, W = np.ascontiguousarray(E[:, :nb]), np.ascontiguousarray(W[:, :nb, :])
+    om = wl.omega_grid(-6.0, 4.0, 4000)
+    ref = oracle.tetra_dos(E, W, nk, om)
+    with binding.Plan(nk, nb, norb, 4000) as plan_a:
+        with binding.Plan(nk, nb, norb, 100) as plan_b:
+            run_gpu(E, W, nk, wl.omega_grid(-6.0, 4.0, 100), plan=plan_b)
+        dos, nos = run_gpu(E, W, nk, om, plan=plan_a)
+        assert_parity(ref, dos, nos, "plan A after plan B")
+
+
+def test_back_to_back_calls_on_two_streams():
+    """A plan's scratch is shared by its calls: a call on another stream waits for the previous call's end, so
+    asynchronous calls issued back to back on two streams give two correct results."""
+    import torch
+    nk, nb, norb, nE = (10, 10, 10), 3, 8, 700
+    E, W = wl.random_bands(nk, nb, norb, seed=23)
+    om = wl.omega_grid(-1.2, 1.3, nE)
+    ref = oracle.tetra_dos(E, W, nk, om)
+    E2 = (E + np.float32(0.125)).astype(np.float32)
+    ref2 = oracle.tetra_dos(E2, W, nk, om)
+    dev = torch.device("cuda:0")
+    dE, dE2, dW, dOm = (torch.from_numpy(a).to(dev) for a in (E, E2, W, om))
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = [(torch.empty((norb, nE), device=dev), torch.empty((norb, nE), device=dev)) for _ in range(4)]
+    torch.cuda.synchronize()
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        for i, (st, e) in enumerate(((s1, dE), (s2, dE2), (s1, dE), (s2, dE2))):
+            plan.tetra_dos(e, dW, dOm, outs[i][0], outs[i][1], stream=st.cuda_stream)
+        torch.cuda.synchronize()
+    for i, r in enumerate((ref, ref2, ref, ref2)):
+        assert_parity(r, outs[i][0].cpu().numpy(), outs[i][1].cpu().numpy(), "two streams, call %d" % i)

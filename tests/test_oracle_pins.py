@@ -408,6 +408,25 @@ def test_P9_invariances_and_variants(oracle_lib):
     assert np.allclose(l2["dos"], w2["dos"], rtol=1e-13, atol=1e-15) and np.allclose(l2["nos"], w2["nos"], rtol=1e-12, atol=1e-14)
 
 
+def test_windowed_oracle_equals_literal_on_configs_1_and_2(oracle_lib, cache_dir):
+    """BASELINE.md 3 / SURVEY.md 8(c) step 5: the windowed variant (skips omega outside (E1, E4), Eq. 15 as step +
+    prefix sum) may stand in for the literal loop at full size only once it reproduces it on the configs the literal
+    loop can afford: config 1 and config 2 (Nk = 32, 8 bands, 8 orbitals, 1000 energies) -- DOS and N to 1e-12
+    relative, equal work counters."""
+    for name in ("cfg1", "cfg2"):
+        cfg = wl.CONFIGS[name]
+        E, W, om = wl.make_inputs(cfg, cache_dir)
+        lit = oracle_lib.tetra_dos(E, W, cfg.nk, om, nthreads=oracle_lib.max_threads())
+        win = oracle_lib.tetra_dos(E, W, cfg.nk, om, windowed=True, nthreads=oracle_lib.max_threads())
+        assert lit["n_eval"] == win["n_eval"] and lit["n_tb"] == win["n_tb"] == 6 * int(np.prod(cfg.nk)) * cfg.nb
+        assert list(lit["n_case"]) == list(win["n_case"])
+        scale_d = np.abs(lit["dos"]).max()
+        assert np.abs(lit["dos"] - win["dos"]).max() <= 1e-12 * scale_d
+        pos = lit["nos"] > 0
+        assert np.array_equal(pos, win["nos"] > 0)
+        assert (np.abs(lit["nos"] - win["nos"])[pos] / lit["nos"][pos]).max() <= 1e-12
+
+
 def test_flat_band_and_grid_outside_bands(oracle_lib):
     """Flat band: DOS = 0 at every omega (delta spike lost, inherent), N = step at e, 0 AT e.
     omega grid entirely below / above the bands: zeros / full count."""
