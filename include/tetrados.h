@@ -115,6 +115,19 @@ int tetra_dos_complex(tdos_plan* p, const float* E, const float* A, int layout, 
                       float* dos, float* nos, int memspace, void* cuda_stream);
 
 /*
+ * Orbital selection plus total ("the five Fe 3d orbitals ... and the total density of states" of an
+ * 8-orbital model; reading G15: total = sum over ALL orbitals).  Rows of dos / nos:
+ *     j < nsel : orbital orbitals[j] (0-based, each < norb, any order, repeats allowed),
+ *     j = nsel : sum over all norb orbitals, present if want_total != 0.
+ * dos, nos are [nsel + (want_total != 0)][nE]; nsel <= 32, at most norb + 1 rows; nsel = 0 with want_total gives the
+ * total alone.  W must not be NULL; `orbitals` is a HOST array in both memory spaces.  Everything else as tetra_dos.
+ * The selection is applied while a tile is staged, so only the rows asked for are projected and accumulated.
+ */
+int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+                     const int* orbitals, int nsel, int want_total, float* dos, float* nos, int memspace,
+                     void* cuda_stream);
+
+/*
  * Multi-GPU building blocks (device pointers only).
  * tetra_dos_partial: the additive share of the cubes with z_lo <= iz < z_hi, as raw fp64 sums
  *   part[3][norb][nE]  (0: sum b*dw/V, 1: sum b*w/V over E1 < omega < E4, 2: Eq.-15 step histogram / V at the first omega >= E4),

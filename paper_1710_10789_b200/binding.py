@@ -17,7 +17,7 @@ TDOS_MAX_NE = 65534
 
 # every symbol include/tetrados.h declares
 SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy",
-           "tetra_dos", "tetra_dos_complex", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
+           "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
            "tdos_last_counters", "tdos_kernel_ms", "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
 
 _lib = None
@@ -51,6 +51,7 @@ def load():
     lib.tdos_plan_destroy.argtypes = [vp]
     lib.tetra_dos.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
     lib.tetra_dos_complex.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
+    lib.tetra_dos_select.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, ip, C.c_int, C.c_int, fp, fp, C.c_int, vp]
     lib.tetra_weights.argtypes = [vp, fp, C.c_int, fp, C.c_int, fp, fp, vp]
     lib.tetra_dos_partial.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, C.c_int, C.c_int, vp, vp]
     lib.tetra_dos_finalize.argtypes = [vp, vp, C.c_int, fp, fp, vp]
@@ -125,6 +126,15 @@ class Plan:
         nE = int(omega.shape[0])
         _check(load().tetra_dos_complex(self._h, _ptr(E), _ptr(A), layout, _ptr(omega), nE, _ptr(dos), _ptr(nos),
                                         memspace, _stream_ptr(stream, memspace)), "tetra_dos_complex")
+
+    def tetra_dos_select(self, E, W, omega, orbitals, want_total: bool, dos, nos=None, layout: int = TDOS_AOS,
+                         memspace: int = TDOS_DEVICE, stream=None):
+        """tetra_dos_select(): rows = the listed orbitals, then (want_total) the sum over all orbitals."""
+        nE = int(omega.shape[0])
+        orb = (C.c_int * max(len(orbitals), 1))(*[int(x) for x in orbitals])
+        _check(load().tetra_dos_select(self._h, _ptr(E), _ptr(W), layout, _ptr(omega), nE, orb, len(orbitals),
+                                       1 if want_total else 0, _ptr(dos), _ptr(nos), memspace,
+                                       _stream_ptr(stream, memspace)), "tetra_dos_select")
 
     def tetra_weights(self, E, energies, wk, dwk=None, layout: int = TDOS_AOS, stream=None):
         """tetra_weights(): per-k-point integration weights wk[nW][nb][nk] (and dwk) for device tensors."""

@@ -44,6 +44,11 @@ struct MainParams {
     int nmb;                     // orbital blocks of MB
     int n_items;                 // ntx*nty*ntz*nb*nmb
     int unitW;                   // W == 1
+    // orbital selection (tetra_dos_select; "five Fe 3d orbitals ... and the total"): nsel > 0 or
+    // total: output row j < nsel is input orbital sel[j], row nsel (if total) is the sum over all norb_in input
+    // orbitals, the rows up to norb are zero padding.  Otherwise output row = input orbital.
+    int nsel, total, norb_in;
+    signed char sel[32];
     int cplx;                    // W holds complex eigenvector elements a (re, im pairs), strides count pairs: b = |a|^2
     int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
     // kernel choice on the device (null: this kernel runs): {sum of window lengths in bins, (tetrahedron, band) pairs}
@@ -73,6 +78,16 @@ __device__ __forceinline__ float load_weight(const MainParams& p, long long idx)
         return fmaf(a.x, a.x, a.y * a.y);
     }
     return __ldg(p.W + idx);
+}
+
+// weight of OUTPUT row j (< p.norb) at the k-point/band whose orbital 0 sits at `base`
+__device__ __forceinline__ float load_out_weight(const MainParams& p, long long base, int j) {
+    if (p.nsel == 0 && !p.total) return load_weight(p, base + (long long)j * p.sWm);
+    if (j < p.nsel) return load_weight(p, base + (long long)p.sel[j] * p.sWm);
+    float s = 0.0f;
+    if (j == p.nsel && p.total)
+        for (int m = 0; m < p.norb_in; m++) s += load_weight(p, base + (long long)m * p.sWm);
+    return s;
 }
 
 // first index i in [0, nE] with omega[i] >= x (STRICT = false) or omega[i] > x (STRICT = true):
@@ -266,7 +281,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     }
     float* part = p.partial + (size_t)blockIdx.x * 3 * norb * p.nEp;   // rows [bin][ D | T | S ]
     const bool vec4 = (MB % 4 == 0) && (norb % 4 == 0);          // 16-byte aligned vector reductions
-    const bool w_vec4 = (MB % 4 == 0) && !p.unitW && !p.cplx && p.sWm == 1 && (norb % 4 == 0) &&
+    const bool w_vec4 = (MB % 4 == 0) && !p.unitW && !p.cplx && p.sWm == 1 && (norb % 4 == 0) && p.nsel == 0 && !p.total &&
                         ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
 
     const int g = lane / GL, gl = lane % GL;
@@ -312,7 +327,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
-                sW[k * WST + m] = (m0 + m < norb) ? load_weight(p, ik * p.sWk + (long long)n * p.sWn + (m0 + m)) : 0.0f;
+                sW[k * WST + m] = (m0 + m < norb) ? load_out_weight(p, ik * p.sWk + (long long)n * p.sWn, m0 + m) : 0.0f;
             }
         } else {                   // k contiguous (SoA): k fastest across lanes
             for (int q = lane; q < PK * MB; q += 32) {
@@ -320,9 +335,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
-                sW[k * WST + m] = (m0 + m < norb)
-                                      ? load_weight(p, ik * p.sWk + (long long)n * p.sWn + (long long)(m0 + m) * p.sWm)
-                                      : 0.0f;
+                sW[k * WST + m] = (m0 + m < norb) ? load_out_weight(p, ik * p.sWk + (long long)n * p.sWn, m0 + m) : 0.0f;
             }
         }
         __syncwarp();

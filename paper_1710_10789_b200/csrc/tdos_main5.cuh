@@ -442,7 +442,8 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
     }
     // rows [bin][ D | T | S ], norb % 4 == 0 (the host picks this kernel only then), nEp = nE rounded up to 4 rows
     float* part = p.partial + (size_t)blockIdx.x * 3 * norb * p.nEp;
-    const bool w_vec4 = !p.unitW && !p.cplx && p.sWm == 1 && ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
+    const bool w_vec4 = !p.unitW && !p.cplx && p.sWm == 1 && p.nsel == 0 && !p.total &&
+                        ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
     float* sOm = reinterpret_cast<float*>(base + C::off_om);
     unsigned long long cnt_tb = 0, cnt_ev = 0, cnt_mid = 0;
 
@@ -492,9 +493,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
                 int gx = x0 + px, gy = y0 + py, gz = z0 + pz;
                 while (gx >= p.N1) gx -= p.N1; while (gy >= p.N2) gy -= p.N2; while (gz >= p.N3) gz -= p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
-                sW[k * WST + m] = (m0 + m < norb)
-                                      ? load_weight(p, ik * p.sWk + (long long)n * p.sWn + (long long)(m0 + m) * p.sWm)
-                                      : 0.0f;
+                sW[k * WST + m] = (m0 + m < norb) ? load_out_weight(p, ik * p.sWk + (long long)n * p.sWn, m0 + m) : 0.0f;
             }
         }
         __syncwarp();

@@ -134,6 +134,12 @@ struct tdos_plan {
     float* dW = nullptr;
     size_t dW_floats = 0;         // capacity of dW
     int cplx = 0;                 // the call in flight passes complex eigenvector elements instead of weights
+    // the call in flight: rows the kernels work on (k_norb: output rows padded for the kernel in use), rows the caller
+    // gets (k_nout), orbital selection (tetra_dos_select)
+    int norb_alloc = 0;           // rows the scratch buffers hold: norb + 1 (selection + total), rounded up to 4
+    int k_norb = 0, k_nout = 0;
+    int sel_n = 0, sel_total = 0;
+    signed char sel[32] = {};
     float* dOm = nullptr;
     float* dDos = nullptr;
     float* dNos = nullptr;
@@ -152,6 +158,13 @@ struct tdos_plan {
     bool timed = false;
     long long last_items = 0, last_launches = 0;
 };
+
+// what a call without orbital selection works on
+static void reset_call_state(tdos_plan* p) {
+    p->cplx = 0;
+    p->k_norb = p->k_nout = p->norb;
+    p->sel_n = p->sel_total = 0;
+}
 
 extern "C" {
 
@@ -212,6 +225,8 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     memcpy(p->nk, nk, sizeof(p->nk));
     p->nb = nb;
     p->norb = norb;
+    p->norb_alloc = (norb + 1 + 3) & ~3;
+    p->k_norb = p->k_nout = norb;
     p->nE_max = nE_max;
     p->num_sms = prop.multiProcessorCount;
     p->smem_optin = prop.sharedMemPerBlockOptin;
@@ -264,7 +279,7 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
         cudaGetLastError();
     }
 
-    const size_t hist = (size_t)3 * norb * ((size_t)nE_max + 3);
+    const size_t hist = (size_t)3 * p->norb_alloc * ((size_t)nE_max + 3);
     if (cudaMalloc(&p->partial, hist * p->nparts * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&p->part64, hist * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&p->counters, 8 * sizeof(unsigned long long)) != cudaSuccess) {
@@ -341,7 +356,9 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         mp.sWk = 1; mp.sWn = (long long)p->norb * nkt; mp.sWm = nkt;
     }
     mp.N1 = p->nk[0]; mp.N2 = p->nk[1]; mp.N3 = p->nk[2];
-    mp.nb = p->nb; mp.norb = p->norb; mp.nE = nE;
+    mp.nb = p->nb; mp.norb = p->k_norb; mp.nE = nE;
+    mp.nsel = p->sel_n; mp.total = p->sel_total; mp.norb_in = p->norb;
+    memcpy(mp.sel, p->sel, sizeof(mp.sel));
     mp.nEp = rows_per_block(nE);
     mp.z_lo = z_lo; mp.z_hi = z_hi;
     mp.unitW = (W == nullptr);
@@ -351,7 +368,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
     mp.est = p->adaptive ? p->counters + 4 : nullptr;
 
-    const size_t hist = (size_t)3 * p->norb * mp.nEp;
+    const size_t hist = (size_t)3 * p->k_norb * mp.nEp;
     if (first) {
         CK(cudaMemsetAsync(p->partial, 0, hist * p->nparts * sizeof(float), st));
         CK(cudaMemsetAsync(p->counters, 0, 8 * sizeof(unsigned long long), st));
@@ -381,7 +398,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         mp.ntx = (p->nk[0] + v.TX - 1) / v.TX;
         mp.nty = (p->nk[1] + v.TY - 1) / v.TY;
         mp.ntz = (z_hi - z_lo + v.TZ - 1) / v.TZ;
-        mp.nmb = (p->norb + v.MB - 1) / v.MB;
+        mp.nmb = (p->k_norb + v.MB - 1) / v.MB;
         const long long items = (long long)mp.ntx * mp.nty * mp.ntz * p->nb * mp.nmb;
         if (items > 0x7fffffffLL) return TDOS_EINVAL;
         mp.n_items = (int)items;
@@ -410,9 +427,9 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
 
 // fp64 sum of the block partials -> part_out (device fp64 [3][norb][nE])
 static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st) {
-    const size_t hist = (size_t)3 * p->norb * nE;
+    const size_t hist = (size_t)3 * p->k_norb * nE;
     const int mblocks = (int)((hist + 255) / 256);
-    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->nparts, p->norb, nE, rows_per_block(nE), part_out);
+    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->nparts, p->k_norb, nE, rows_per_block(nE), part_out);
     CK(cudaGetLastError());
     p->last_launches += 1;
     return TDOS_OK;
@@ -432,7 +449,7 @@ static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int lay
 
 static int enqueue_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos, cudaStream_t st) {
     const double V = 1.0 / (24.0 * (double)p->nk[0] * (double)p->nk[1] * (double)p->nk[2]);
-    tdos::tdos_finalize<<<p->norb, 1024, 0, st>>>(part, p->norb, nE, V, dos, nos);
+    tdos::tdos_finalize<<<p->k_nout, 1024, 0, st>>>(part, p->k_norb, nE, V, dos, nos);
     CK(cudaGetLastError());
     p->last_launches += 1;
     return TDOS_OK;
@@ -444,6 +461,7 @@ int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, 
     if (rc) return rc;
     if (!part || z_lo < 0 || z_hi > p->nk[2] || z_lo > z_hi) return TDOS_EINVAL;
     ON_DEVICE(p->device);
+    reset_call_state(p);
     p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
     rc = enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream);
     if (rc) return rc;
@@ -456,6 +474,7 @@ int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, 
 int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos, void* cuda_stream) {
     if (!p || !part || !dos || nE < 1 || nE > p->nE_max) return TDOS_EINVAL;
     ON_DEVICE(p->device);
+    reset_call_state(p);
     return enqueue_finalize(p, part, nE, dos, nos, (cudaStream_t)cuda_stream);
 }
 
@@ -477,13 +496,34 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
 
 int tetra_dos(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE, float* dos,
               float* nos, int memspace, void* cuda_stream) {
-    if (p) p->cplx = 0;
+    if (p) reset_call_state(p);
     return tetra_dos_impl(p, E, W, layout, omega, nE, dos, nos, memspace, cuda_stream);
+}
+
+int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+                     const int* orbitals, int nsel, int want_total, float* dos, float* nos, int memspace, void* cuda_stream) {
+    if (!p || !W || nsel < 0 || nsel > 32 || (nsel > 0 && !orbitals) || (nsel == 0 && !want_total)) return TDOS_EINVAL;
+    for (int j = 0; j < nsel; j++)
+        if (orbitals[j] < 0 || orbitals[j] >= p->norb) return TDOS_EINVAL;
+    reset_call_state(p);
+    const int nout = nsel + (want_total ? 1 : 0);
+    if (nout > p->norb + 1) return TDOS_EINVAL;   // the scratch buffers hold norb + 1 rows
+    p->sel_n = nsel;
+    p->sel_total = want_total ? 1 : 0;
+    for (int j = 0; j < nsel; j++) p->sel[j] = (signed char)orbitals[j];
+    p->k_nout = nout;
+    // generation 5 works on whole blocks of 4 orbitals, at least 5 rows: the selection is padded with zero rows
+    p->k_norb = (p->var.gen == 5) ? (nout <= 8 ? 8 : (nout + 3) & ~3) : nout;
+    if (p->k_norb > p->norb_alloc) p->k_norb = p->norb_alloc;   // (norb_alloc = norb + 1 rounded up to 4 >= 8 for generation 5)
+    const int rc = tetra_dos_impl(p, E, W, layout, omega, nE, dos, nos, memspace, cuda_stream);
+    reset_call_state(p);
+    return rc;
 }
 
 int tetra_dos_complex(tdos_plan* p, const float* E, const float* A, int layout, const float* omega, int nE,
                       float* dos, float* nos, int memspace, void* cuda_stream) {
     if (!p || !A) return TDOS_EINVAL;
+    reset_call_state(p);
     p->cplx = 1;
     const int rc = tetra_dos_impl(p, E, A, layout, omega, nE, dos, nos, memspace, cuda_stream);
     p->cplx = 0;
@@ -521,8 +561,8 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
         p->dW_floats = nkt * p->nb * p->norb * wfl;
         if (cudaMalloc(&p->dE, nkt * p->nb * sizeof(float)) != cudaSuccess ||
             cudaMalloc(&p->dW, p->dW_floats * sizeof(float)) != cudaSuccess ||
-            cudaMalloc(&p->dOm, nEb) != cudaSuccess || cudaMalloc(&p->dDos, nEb * p->norb) != cudaSuccess ||
-            cudaMalloc(&p->dNos, nEb * p->norb) != cudaSuccess) {
+            cudaMalloc(&p->dOm, nEb) != cudaSuccess || cudaMalloc(&p->dDos, nEb * (p->norb + 1)) != cudaSuccess ||
+            cudaMalloc(&p->dNos, nEb * (p->norb + 1)) != cudaSuccess) {
             cudaGetLastError();
             cudaFree(p->dE); cudaFree(p->dW); cudaFree(p->dOm); cudaFree(p->dDos); cudaFree(p->dNos);
             p->dE = p->dW = p->dOm = p->dDos = p->dNos = nullptr;
@@ -606,8 +646,8 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
     CK(cudaEventRecord(p->ring[p->cur_slot][2], st));
     p->n_timed_calls++;
     p->timed = true;
-    CK(cudaMemcpyAsync(dos, p->dDos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
-    if (nos) CK(cudaMemcpyAsync(nos, p->dNos, (size_t)p->norb * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(dos, p->dDos, (size_t)p->k_nout * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (nos) CK(cudaMemcpyAsync(nos, p->dNos, (size_t)p->k_nout * nE * sizeof(float), cudaMemcpyDeviceToHost, st));
     rc = mark_end_of_call(p, st);
     if (rc) return rc;
     CK(cudaStreamSynchronize(st));

@@ -458,3 +458,63 @@ def test_back_to_back_calls_on_two_streams():
         torch.cuda.synchronize()
     for i, r in enumerate((ref, ref2, ref, ref2)):
         assert_parity(r, outs[i][0].cpu().numpy(), outs[i][1].cpu().numpy(), "two streams, call %d" % i)
+
+
+@pytest.mark.parametrize("host", [False, True])
+def test_orbital_selection_plus_total_paper_shape(cache_dir, host):
+    """five selected orbitals of the 8-orbital model and the total DOS on the
+    paper's 60 x 60 x 10 grid with 1024 energies.  Rows 0..4 must equal the oracle's rows of those orbitals, row 5 the
+    sum over all eight (reading G15; linear in W, so the oracle's rows add up to it)."""
+    cfg = wl.CONFIGS["paper60"]
+    E, W, om, ref = _full_ref("paper60", cache_dir)
+    sel = [0, 2, 3, 5, 7]
+    want = {"dos": np.concatenate([ref["dos"][sel], ref["dos"].sum(axis=0, keepdims=True)]),
+            "nos": np.concatenate([ref["nos"][sel], ref["nos"].sum(axis=0, keepdims=True)])}
+    import torch
+    with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
+        if host:
+            dos, nos = np.full((6, cfg.nE), np.nan, np.float32), np.full((6, cfg.nE), np.nan, np.float32)
+            plan.tetra_dos_select(E, W, om, sel, True, dos, nos, memspace=binding.TDOS_HOST)
+        else:
+            dev = torch.device("cuda:0")
+            dE, dW, dOm = (torch.from_numpy(a).to(dev) for a in (E, W, om))
+            ddos = torch.full((6, cfg.nE), float("nan"), device=dev)
+            dnos = torch.full((6, cfg.nE), float("nan"), device=dev)
+            plan.tetra_dos_select(dE, dW, dOm, sel, True, ddos, dnos)
+            torch.cuda.synchronize()
+            dos, nos = ddos.cpu().numpy(), dnos.cpu().numpy()
+        assert plan.last_counters()["kernel"] == 5      # the selection stays on the 8-row kernel
+        assert_parity(want, dos, nos, "5 orbitals + total")
+        # a full call on the same plan afterwards is not affected by the selection
+        dos8, nos8 = run_gpu(E, W, cfg.nk, om, plan=plan)
+        assert_parity(ref, dos8, nos8, "full call after a selection")
+
+
+def test_orbital_selection_small_cases():
+    """total alone, repeats and order, SoA, fewer than five rows on a narrow plan (generation 3), norb = 12 with total."""
+    import torch
+    dev = torch.device("cuda:0")
+    for nk, nb, norb, sel, total in (((7, 6, 5), 2, 8, [], True), ((7, 6, 5), 2, 8, [6, 1, 1], False),
+                                     ((5, 4, 6), 3, 3, [2, 0], True), ((4, 5, 3), 2, 12, [11, 0, 4, 5, 6, 7, 8, 9, 10], True)):
+        nE = 300
+        E, W = wl.random_bands(nk, nb, norb, seed=5 + norb)
+        om = wl.omega_grid(-1.2, 1.3, nE)
+        ref = oracle.tetra_dos(E, W, nk, om)
+        rows = [ref["dos"][sel]] + ([ref["dos"].sum(axis=0, keepdims=True)] if total else [])
+        rown = [ref["nos"][sel]] + ([ref["nos"].sum(axis=0, keepdims=True)] if total else [])
+        want = {"dos": np.concatenate(rows), "nos": np.concatenate(rown)}
+        nout = len(sel) + int(total)
+        for layout in (binding.TDOS_AOS, binding.TDOS_SOA):
+            Ex, Wx = (E, W) if layout == binding.TDOS_AOS else wl.to_soa(E, W)
+            dE, dW, dOm = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (Ex, Wx, om))
+            ddos = torch.full((nout, nE), float("nan"), device=dev)
+            dnos = torch.full((nout, nE), float("nan"), device=dev)
+            with binding.Plan(nk, nb, norb, nE) as plan:
+                plan.tetra_dos_select(dE, dW, dOm, sel, total, ddos, dnos, layout=layout)
+                torch.cuda.synchronize()
+            assert_parity(want, ddos.cpu().numpy(), dnos.cpu().numpy(), "select %s total %s norb %d" % (sel, total, norb))
+    with binding.Plan((4, 4, 4), 2, 8, 10) as plan:
+        with pytest.raises(binding.TdosError):
+            plan.tetra_dos_select(dE, dW, dOm, [8], False, ddos, dnos)        # orbital out of range
+        with pytest.raises(binding.TdosError):
+            plan.tetra_dos_select(dE, dW, dOm, [], False, ddos, dnos)         # nothing asked for
