@@ -70,6 +70,7 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-fp64", action="store_true", help="skip the fp64-accumulation variant's cost")
     ap.add_argument("--cache", default=os.environ.get("TDOS_CACHE", "/tmp/tdos_cache"))
     return ap.parse_args()
 
@@ -346,6 +347,24 @@ def main():
                "note": "h2d_gbs = staged bytes / whole e2e step (copies overlapped with the kernels); h2d_gbs_plain = one "
                        "plain cudaMemcpyAsync of the same E + W bytes from the same pinned buffers, timed alone"}
 
+    # ---- cost of the fp64-accumulation variant on the same workload
+    fp64_acc = None
+    if world == 1 and not args.no_fp64:
+        plan.set_accumulation(True)
+        for _ in range(2):
+            step()
+        torch.cuda.synchronize()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        for _ in range(3):
+            step()
+        f1.record()
+        torch.cuda.synchronize()
+        fp64_acc = {"ms_per_step": f0.elapsed_time(f1) / 3, "main_kernel_ms": plan.kernel_ms(3)[0],
+                    "what": "tdos_plan_set_accumulation(TDOS_ACC_FP64): single-precision corner weights, every sum after "
+                            "them in fp64 (generation 3 kernel, fp64 block partials)"}
+        plan.set_accumulation(False)
+
     # ---- roofline of the dominant kernel (tdos_main): FP32 ALU
     props = torch.cuda.get_device_properties(dev)
     sm_max = clocks.get("sm_max_mhz") or 1965.0
@@ -386,6 +405,7 @@ def main():
         "effective_evals_per_s": n_eval / (ms_per_step * 1e-3), "dos_grids_per_s": 1e3 / ms_per_step,
         "n_tb": n_tb, "n_eval": n_eval, "n_eval_mid": n_mid if gen >= 4 else None, "kernel_generation": gen,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
+        "fp64_accumulation": fp64_acc,
     }
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

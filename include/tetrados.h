@@ -82,6 +82,18 @@ const char* tdos_last_cuda_error(void);
  */
 int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int norb, int nE_max);
 
+/*
+ * Precision of the accumulation (Sec. III.B: single precision throughout, "one can in principle switch
+ * to double precision").  TDOS_ACC_FP32 (default): fp32 sums in registers and block partials, fp64 merge and prefix sum.
+ * TDOS_ACC_FP64: the corner weights are still evaluated in single precision, but every sum taken after them (registers,
+ * block partials, the Eq.-15 step histogram, merge, prefix sum) is fp64; slower (about 3x on config 4), results agree
+ * with the fp64 oracle to ~1e-7 relative instead of ~1e-6.  Allocates a second, fp64 set of block
+ * partials the first time the mode is chosen (TDOS_ENOMEM if that fails); waits for the plan's last call.
+ */
+#define TDOS_ACC_FP32 0
+#define TDOS_ACC_FP64 1
+int tdos_plan_set_accumulation(tdos_plan* p, int mode);
+
 /* Free a plan and everything it owns.  NULL is a no-op.  Synchronises the plan's streams first. */
 int tdos_plan_destroy(tdos_plan* p);
 

@@ -12,11 +12,12 @@ from . import build as _build
 
 TDOS_OK, TDOS_EINVAL, TDOS_ENOMEM, TDOS_ECUDA, TDOS_EARCH = 0, -1, -2, -3, -4
 TDOS_AOS, TDOS_SOA = 0, 1
+TDOS_ACC_FP32, TDOS_ACC_FP64 = 0, 1
 TDOS_DEVICE, TDOS_HOST = 0, 1
 TDOS_MAX_NE = 65534
 
 # every symbol include/tetrados.h declares
-SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy",
+SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy", "tdos_plan_set_accumulation",
            "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
            "tdos_last_counters", "tdos_kernel_ms", "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
 
@@ -49,6 +50,7 @@ def load():
     lib.tdos_last_cuda_error.restype = C.c_char_p
     lib.tdos_plan_create.argtypes = [C.POINTER(vp), C.c_int, ip, C.c_int, C.c_int, C.c_int]
     lib.tdos_plan_destroy.argtypes = [vp]
+    lib.tdos_plan_set_accumulation.argtypes = [vp, C.c_int]
     lib.tetra_dos.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
     lib.tetra_dos_complex.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
     lib.tetra_dos_select.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, ip, C.c_int, C.c_int, fp, fp, C.c_int, vp]
@@ -92,6 +94,10 @@ class Plan:
         arr = (C.c_int * 3)(*self.nk)
         _check(lib.tdos_plan_create(C.byref(self._h), self.device, arr, self.nb, self.norb, self.nE_max),
                "tdos_plan_create")
+
+    def set_accumulation(self, fp64: bool):
+        """tdos_plan_set_accumulation(): fp64 sums after the single-precision corner weights."""
+        _check(load().tdos_plan_set_accumulation(self._h, TDOS_ACC_FP64 if fp64 else TDOS_ACC_FP32), "tdos_plan_set_accumulation")
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -27,6 +27,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "tdos_weights.cuh"
 
 namespace tdos {
@@ -55,6 +57,7 @@ struct MainParams {
     // of a sample, written by tdos_estimate earlier on the stream; see wanted_generation()
     const unsigned long long* est;
     float* partial;              // [gridDim.x] rows [nEp][ D(norb) | T(norb) | S(norb) ]
+    double* partial64;           // the same in fp64 (tdos_main<..., ACC64 = true>: "switch to double precision")
     unsigned int* next_item;        // tdos_main5: work counter, zero at launch
     unsigned long long* counters;   // [0] n_tb, [1] n_eval = #(tb, omega) with E1 < omega < E4
 };
@@ -246,7 +249,53 @@ struct Acc {
     }
 };
 
-template <int MB, int TX, int TY, int TZ, int GL, int NWARP>
+// fp64 accumulation ("one can in principle switch to double precision"): the corner weights stay the
+// paper's single-precision arithmetic, every SUM taken after them -- registers, block partials, step histogram,
+// merge -- is fp64.  Same interface as Acc<MB>.
+__device__ __forceinline__ void red_add_f64(double* addr, double v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(v) : "memory");
+}
+template <int MB>
+struct Acc64 {
+    double D[2][MB], T[2][MB];
+    __device__ __forceinline__ void zero() {
+#pragma unroll
+        for (int h = 0; h < 2; h++)
+#pragma unroll
+            for (int m = 0; m < MB; m++) D[h][m] = T[h][m] = 0.0;
+    }
+    __device__ __forceinline__ void project(const float* __restrict__ sW, const unsigned (&cc)[4], const f2 (&w)[4],
+                                            const f2 (&dw)[4]) {
+#pragma unroll
+        for (int l = 0; l < 4; l++) {
+            float b[MB];
+            load_b<MB>(sW + cc[l], b);
+            const double da = (double)dw[l].x, db = (double)dw[l].y, wa = (double)w[l].x, wb = (double)w[l].y;
+#pragma unroll
+            for (int m = 0; m < MB; m++) {
+                const double bm = (double)b[m];
+                D[0][m] = fma(bm, da, D[0][m]);
+                D[1][m] = fma(bm, db, D[1][m]);
+                T[0][m] = fma(bm, wa, T[0][m]);
+                T[1][m] = fma(bm, wb, T[1][m]);
+            }
+        }
+    }
+    __device__ __forceinline__ void flush(double* __restrict__ part, int bin0, int nE, int norb, int m0, bool) {
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            if (bin0 + h < nE) {
+                double* row = part + (size_t)(bin0 + h) * 3 * norb + m0;
+#pragma unroll
+                for (int m = 0; m < MB; m++)
+                    if (m0 + m < norb) { red_add_f64(row + m, D[h][m]); red_add_f64(row + norb + m, T[h][m]); }
+            }
+        }
+        zero();
+    }
+};
+
+template <int MB, int TX, int TY, int TZ, int GL, int NWARP, bool ACC64 = false>
 __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     using Cfg = WarpCfg<MB, TX, TY, TZ>;
     constexpr int PX = Cfg::PX, PY = Cfg::PY, PK = Cfg::PK, NC = Cfg::NC, NTB = Cfg::NTB;
@@ -279,7 +328,11 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
         const float span = __ldg(omega + nE - 1) - om0;
         if (span > 0.0f) inv_dom = (float)(nE - 1) / span;
     }
-    float* part = p.partial + (size_t)blockIdx.x * 3 * norb * p.nEp;   // rows [bin][ D | T | S ]
+    // rows [bin][ D | T | S ] of this block's partial histogram, fp32 or (ACC64) fp64
+    using part_t = typename std::conditional<ACC64, double, float>::type;
+    part_t* part;
+    if constexpr (ACC64) part = p.partial64 + (size_t)blockIdx.x * 3 * norb * p.nEp;
+    else part = p.partial + (size_t)blockIdx.x * 3 * norb * p.nEp;
     const bool vec4 = (MB % 4 == 0) && (norb % 4 == 0);          // 16-byte aligned vector reductions
     const bool w_vec4 = (MB % 4 == 0) && !p.unitW && !p.cplx && p.sWm == 1 && (norb % 4 == 0) && p.nsel == 0 && !p.total &&
                         ((reinterpret_cast<uintptr_t>(p.W) & 15) == 0);
@@ -389,8 +442,13 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                         load_b<MB>(sW + c1, b1);
                         load_b<MB>(sW + c2, b2);
                         load_b<MB>(sW + c3, b3);
-                        float* dst = part + (size_t)i4 * 3 * norb + 2 * norb + m0;
-                        if (vec4) {
+                        part_t* dst = part + (size_t)i4 * 3 * norb + 2 * norb + m0;
+                        if constexpr (ACC64) {
+#pragma unroll
+                            for (int m = 0; m < MB; m++)
+                                if (m0 + m < norb)
+                                    red_add_f64(dst + m, ((double)b0[m] + (double)b1[m]) + ((double)b2[m] + (double)b3[m]));
+                        } else if (vec4) {
                             if constexpr (MB % 4 == 0) {
 #pragma unroll
                                 for (int m4 = 0; m4 < MB; m4 += 4)
@@ -487,7 +545,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
             int bin0 = pb + c * CH + 2 * gl;
             f2 om = make_float2((bin0 < nE) ? __ldg(omega + bin0) : qnan, (bin0 + 1 < nE) ? __ldg(omega + bin0 + 1) : qnan);
 
-            Acc<MB> acc;
+            typename std::conditional<ACC64, Acc64<MB>, Acc<MB>>::type acc;
             acc.zero();
 
             // -- A4-A6: every group walks its share of the list; lanes own bins
@@ -601,6 +659,18 @@ __global__ void __launch_bounds__(256) tdos_merge(const float* __restrict__ part
     for (size_t j = blockIdx.x * (size_t)blockDim.x + threadIdx.x; j < n; j += (size_t)gridDim.x * blockDim.x) {
         double s = 0.0;
         for (int c = 0; c < nblk; c++) s += (double)partial[(size_t)c * bstride + j];
+        const size_t i = j / (3 * norb), qm = j - i * (3 * norb);
+        out[qm * nE + i] = s;
+    }
+}
+
+// A7a for fp64 partials
+__global__ void __launch_bounds__(256) tdos_merge64(const double* __restrict__ partial, int nblk, int norb, int nE, int nEp,
+                                                    double* __restrict__ out) {
+    const size_t n = (size_t)3 * norb * nE, bstride = (size_t)3 * norb * nEp;
+    for (size_t j = blockIdx.x * (size_t)blockDim.x + threadIdx.x; j < n; j += (size_t)gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int c = 0; c < nblk; c++) s += partial[(size_t)c * bstride + j];
         const size_t i = j / (3 * norb), qm = j - i * (3 * norb);
         out[qm * nE + i] = s;
     }

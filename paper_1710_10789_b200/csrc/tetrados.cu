@@ -88,6 +88,22 @@ Variant make_variant() {
                    (size_t)NWARP * tdos::WarpCfg<MB, TX, TY, TZ>::bytes};
 }
 
+// fp64 accumulation (tdos_plan_set_accumulation): generation 3 with double-precision registers and partials; 12 warps
+// leave room for the 64 accumulator registers of a block of 8 orbitals
+template <int MB>
+Variant make_variant64() {
+    Variant v{tdos::tdos_main<MB, 4, 4, 2, 2, 12, true>, MB, 4, 4, 2, 2, 12, (size_t)12 * tdos::WarpCfg<MB, 4, 4, 2>::bytes};
+    return v;
+}
+Variant variant64(int MB) {
+    switch (MB) {
+        case 1: return make_variant64<1>();
+        case 2: return make_variant64<2>();
+        case 4: return make_variant64<4>();
+        default: return make_variant64<8>();
+    }
+}
+
 // orbital-block width: the smallest of 1, 2, 4, 8 that holds norb (8 for norb > 8, several blocks)
 int pick_mb(int norb) { return norb <= 1 ? 1 : norb <= 2 ? 2 : norb <= 4 ? 4 : 8; }
 
@@ -119,6 +135,10 @@ struct tdos_plan {
     Variant var{};                // the main kernel (generation 5 when the orbitals allow it, else 3)
     Variant var_short{};          // adaptive plans: generation 3, better when the windows are a few bins only
     bool adaptive = false;        // both kernels are enqueued; the device picks one per call (tdos_estimate)
+    bool acc64 = false;           // tdos_plan_set_accumulation(TDOS_ACC_FP64): var64 runs, partials in fp64
+    Variant var64{};
+    int grid64 = 0;
+    double* partial64 = nullptr;  // [grid64] rows [nE_max + 3][3 * norb_alloc], allocated when the mode is first set
     int blocks_per_sm = 0;
     int grid = 0;                 // blocks of `var`
     int grid_short = 0;           // blocks of `var_short`
@@ -189,6 +209,7 @@ int tdos_plan_destroy(tdos_plan* p) {
     if (p->side) cudaStreamSynchronize(p->side);
     if (p->main) cudaStreamSynchronize(p->main);
     cudaFree(p->partial);
+    cudaFree(p->partial64);
     cudaFree(p->part64);
     cudaFree(p->counters);
     cudaFree(p->dE);
@@ -366,15 +387,18 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     mp.partial = p->partial;
     mp.counters = p->counters;
     mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
-    mp.est = p->adaptive ? p->counters + 4 : nullptr;
+    mp.partial64 = p->partial64;
+    const bool pair = p->adaptive && !p->acc64;   // both kernels enqueued, the device picks
+    mp.est = pair ? p->counters + 4 : nullptr;
 
     const size_t hist = (size_t)3 * p->k_norb * mp.nEp;
     if (first) {
-        CK(cudaMemsetAsync(p->partial, 0, hist * p->nparts * sizeof(float), st));
+        if (p->acc64) CK(cudaMemsetAsync(p->partial64, 0, hist * p->grid64 * sizeof(double), st));
+        else CK(cudaMemsetAsync(p->partial, 0, hist * p->nparts * sizeof(float), st));
         CK(cudaMemsetAsync(p->counters, 0, 8 * sizeof(unsigned long long), st));
         p->last_items = 0;
         p->last_launches = 0;
-        if (p->adaptive && z_hi > z_lo) {   // sample the windows of this call's (first) slab: the device picks the kernel
+        if (pair && z_hi > z_lo) {   // sample the windows of this call's (first) slab: the device picks the kernel
             tdos::EstimateParams ep{};
             ep.E = E; ep.omega = omega;
             ep.sEk = mp.sEk; ep.sEn = mp.sEn;
@@ -392,9 +416,9 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         CK(cudaMemsetAsync(p->counters + 3, 0, sizeof(unsigned long long), st));
     }
     long long items_main = 0;
-    for (int which = 0; which < (p->adaptive ? 2 : 1); ++which) {
-        const Variant& v = which ? p->var_short : p->var;
-        const int vgrid = which ? p->grid_short : p->grid;
+    for (int which = 0; which < (pair ? 2 : 1); ++which) {
+        const Variant& v = p->acc64 ? p->var64 : which ? p->var_short : p->var;
+        const int vgrid = p->acc64 ? p->grid64 : which ? p->grid_short : p->grid;
         mp.ntx = (p->nk[0] + v.TX - 1) / v.TX;
         mp.nty = (p->nk[1] + v.TY - 1) / v.TY;
         mp.ntz = (z_hi - z_lo + v.TZ - 1) / v.TZ;
@@ -429,7 +453,10 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
 static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st) {
     const size_t hist = (size_t)3 * p->k_norb * nE;
     const int mblocks = (int)((hist + 255) / 256);
-    tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->nparts, p->k_norb, nE, rows_per_block(nE), part_out);
+    if (p->acc64)
+        tdos::tdos_merge64<<<mblocks, 256, 0, st>>>(p->partial64, p->grid64, p->k_norb, nE, rows_per_block(nE), part_out);
+    else
+        tdos::tdos_merge<<<mblocks, 256, 0, st>>>(p->partial, p->nparts, p->k_norb, nE, rows_per_block(nE), part_out);
     CK(cudaGetLastError());
     p->last_launches += 1;
     return TDOS_OK;
@@ -513,7 +540,7 @@ int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, c
     for (int j = 0; j < nsel; j++) p->sel[j] = (signed char)orbitals[j];
     p->k_nout = nout;
     // generation 5 works on whole blocks of 4 orbitals, at least 5 rows: the selection is padded with zero rows
-    p->k_norb = (p->var.gen == 5) ? (nout <= 8 ? 8 : (nout + 3) & ~3) : nout;
+    p->k_norb = (p->var.gen == 5 && !p->acc64) ? (nout <= 8 ? 8 : (nout + 3) & ~3) : nout;
     if (p->k_norb > p->norb_alloc) p->k_norb = p->norb_alloc;   // (norb_alloc = norb + 1 rounded up to 4 >= 8 for generation 5)
     const int rc = tetra_dos_impl(p, E, W, layout, omega, nE, dos, nos, memspace, cuda_stream);
     reset_call_state(p);
@@ -705,6 +732,29 @@ int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, f
     return rc;
 }
 
+int tdos_plan_set_accumulation(tdos_plan* p, int mode) {
+    if (!p || (mode != TDOS_ACC_FP32 && mode != TDOS_ACC_FP64)) return TDOS_EINVAL;
+    ON_DEVICE(p->device);
+    if (mode == TDOS_ACC_FP64 && !p->partial64) {
+        p->var64 = variant64(pick_mb(p->norb));
+        int bps = 0;
+        cudaError_t e = cudaFuncSetAttribute((const void*)p->var64.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_optin);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)p->var64.fn, p->var64.NWARP * 32, p->var64.smem);
+        if (e != cudaSuccess || bps < 1) return (e != cudaSuccess) ? cuda_fail(e, "kernel setup") : TDOS_ECUDA;
+        p->grid64 = p->num_sms * bps;
+        const size_t hist = (size_t)3 * p->norb_alloc * ((size_t)p->nE_max + 3);
+        if (cudaMalloc(&p->partial64, hist * p->grid64 * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            p->partial64 = nullptr;
+            return TDOS_ENOMEM;
+        }
+    }
+    if (p->last_stream_valid) CK(cudaStreamSynchronize(p->last_stream));   // no call in flight changes its kernels
+    p->acc64 = (mode == TDOS_ACC_FP64);
+    return TDOS_OK;
+}
+
 int tdos_plan_info(const tdos_plan* p, long long what[8]) {
     if (!p || !what) return TDOS_EINVAL;
     what[0] = p->grid;
@@ -724,7 +774,7 @@ int tdos_last_counters(tdos_plan* p, long long cnt[4]) {
     CK(cudaStreamSynchronize(p->last_stream));
     unsigned long long h[6];
     CK(cudaMemcpy(h, p->counters, sizeof(h), cudaMemcpyDeviceToHost));
-    const int gen = p->adaptive ? tdos::wanted_generation(h[4], h[5]) : p->var.gen;   // what the device decided
+    const int gen = p->acc64 ? 3 : p->adaptive ? tdos::wanted_generation(h[4], h[5]) : p->var.gen;   // what the device decided
     cnt[0] = (long long)h[0];
     cnt[1] = (long long)h[1];
     cnt[2] = gen == 5 ? (long long)h[2] : -1;

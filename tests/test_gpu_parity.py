@@ -518,3 +518,58 @@ def test_orbital_selection_small_cases():
             plan.tetra_dos_select(dE, dW, dOm, [8], False, ddos, dnos)        # orbital out of range
         with pytest.raises(binding.TdosError):
             plan.tetra_dos_select(dE, dW, dOm, [], False, ddos, dnos)         # nothing asked for
+
+
+def test_fp64_accumulation_reaches_the_output_rounding_floor(cache_dir):
+    """with tdos_plan_set_accumulation(TDOS_ACC_FP64) the single-precision corner
+    weights are summed in fp64 everywhere.  On the band-structure configs the result then agrees with the fp64 oracle to
+    the rounding of the fp32 OUTPUT arrays (6e-8): tolerance 1.5e-7 on both DOS and N, tighter than the fp32 mode reaches
+    (2e-7 .. 3e-7 on N); switching back restores the default kernels."""
+    for name in ("cfg2", "cfg3"):
+        cfg = wl.CONFIGS[name]
+        E, W, om, ref = _full_ref(name, cache_dir)
+        with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
+            plan.set_accumulation(True)
+            dos, nos = run_gpu(E, W, cfg.nk, om, plan=plan)
+            cnt = plan.last_counters()
+            d64, n64, zero_ok = errors(ref, dos, nos)
+            assert cnt["kernel"] == 3 and cnt["n_tb"] == ref["n_tb"] and cnt["n_eval"] == ref["n_eval"]
+            assert zero_ok and d64 <= 1.5e-7 and n64 <= 1.5e-7, (name, d64, n64)
+            dos_h, nos_h = run_gpu(E, W, cfg.nk, om, plan=plan, memspace=binding.TDOS_HOST)
+            dh, nh, _ = errors(ref, dos_h, nos_h)
+            assert dh <= 1.5e-7 and nh <= 1.5e-7
+            plan.set_accumulation(False)
+            dos, nos = run_gpu(E, W, cfg.nk, om, plan=plan)
+            d32, n32 = assert_parity(ref, dos, nos, name + " fp32 again")
+            assert plan.last_counters()["kernel"] == 5
+            assert n64 < n32
+        print("%s fp64 accumulation dDOS %.2e dN %.2e (fp32: %.2e %.2e)" % (name, d64, n64, d32, n32))
+
+
+@pytest.mark.parametrize("nk,nb,norb,nE", [((5, 3, 7), 3, 8, 333), ((6, 5, 4), 2, 3, 200), ((4, 4, 5), 2, 12, 150), ((3, 4, 3), 1, 1, 64)])
+def test_fp64_accumulation_on_unstructured_energies(nk, nb, norb, nE):
+    """every orbital-block width, selection + total, W = NULL: north-star tolerances (the error left is that of the
+    single-precision weights at nearly degenerate tetrahedra), and never worse than 1.2 x the fp32 mode"""
+    E, W = wl.random_bands(nk, nb, norb, seed=41 + norb)
+    if norb == 1:
+        W = None
+    om = wl.omega_grid(-1.1, 1.2, nE)
+    ref = oracle.tetra_dos(E, W, nk, om)
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        dos, nos = run_gpu(E, W, nk, om, plan=plan)
+        d32, n32 = assert_parity(ref, dos, nos, "fp32")
+        plan.set_accumulation(True)
+        dos, nos = run_gpu(E, W, nk, om, plan=plan)
+        d64, n64 = assert_parity(ref, dos, nos, "fp64")
+        assert n64 <= 1.2 * n32 + 1e-9 and d64 <= 1.2 * d32 + 1e-9
+        if norb >= 3:
+            import torch
+            dev = torch.device("cuda:0")
+            dE, dW, dOm = (torch.from_numpy(a).to(dev) for a in (E, W, om))
+            ddos = torch.full((3, nE), float("nan"), device=dev)
+            dnos = torch.full((3, nE), float("nan"), device=dev)
+            plan.tetra_dos_select(dE, dW, dOm, [2, 0], True, ddos, dnos)
+            torch.cuda.synchronize()
+            want = {"dos": np.concatenate([ref["dos"][[2, 0]], ref["dos"].sum(axis=0, keepdims=True)]),
+                    "nos": np.concatenate([ref["nos"][[2, 0]], ref["nos"].sum(axis=0, keepdims=True)])}
+            assert_parity(want, ddos.cpu().numpy(), dnos.cpu().numpy(), "fp64 select")
