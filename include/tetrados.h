@@ -140,6 +140,20 @@ int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, c
                      void* cuda_stream);
 
 /*
+ * The step before the path, on the device (Eq. 1, :37-39: the tight-binding Hamiltonian H(k) is "diagonalised
+ * to obtain band energies E_n(k) and eigenvector elements a_n^m(k)"; :289: the best case is input that already
+ * resides in GPU memory): batched Hermitian eigensolver for plans with nb == norb <= 8 (the paper's model: 8).
+ *   H  in  device, nk*nb*nb complex numbers as (re, im) float pairs, H[ik][i][j] row-major, Hermitian
+ *   E  out device [nk][nb], ascending per k-point                                     (TDOS_AOS layout of tetra_dos)
+ *   A  out device [nk][nb][nb][2]: A[ik][n][m] = a_n^m(k), component m of eigenvector n (TDOS_AOS layout of
+ *      tetra_dos_complex), normalised, phase arbitrary
+ * so that  tetra_eigh(p, H, E, A, s); tetra_dos_complex(p, E, A, TDOS_AOS, ...)  goes from H(k) to the DOS without a
+ * host round trip.  Cyclic Jacobi, fp64 arithmetic like the host LAPACK call it replaces, results rounded to the fp32
+ * arrays the path consumes.  Asynchronous on `cuda_stream`.  TDOS_EINVAL if nb != norb or nb > 8.
+ */
+int tetra_eigh(tdos_plan* p, const float* H, float* E, float* A, void* cuda_stream);
+
+/*
  * Multi-GPU building blocks (device pointers only).
  * tetra_dos_partial: the additive share of the cubes with z_lo <= iz < z_hi, as raw fp64 sums
  *   part[3][norb][nE]  (0: sum b*dw/V, 1: sum b*w/V over E1 < omega < E4, 2: Eq.-15 step histogram / V at the first omega >= E4),

@@ -4,6 +4,6 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 legs may import this package.  It shares nothing with paper_1710_10789_b200/.
 """
 from .oracle import (  # noqa: F401
-    build, corner_weights, sort4, table_I, corner_offset, tetra_dos, tetra_weights, max_threads,
+    build, corner_weights, sort4, table_I, corner_offset, tetra_dos, tetra_weights, eigh_bands, max_threads,
     AOS, SOA,
 )

@@ -18,7 +18,7 @@ TDOS_MAX_NE = 65534
 
 # every symbol include/tetrados.h declares
 SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy", "tdos_plan_set_accumulation",
-           "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
+           "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_eigh", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
            "tdos_last_counters", "tdos_kernel_ms", "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
 
 _lib = None
@@ -54,6 +54,7 @@ def load():
     lib.tetra_dos.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
     lib.tetra_dos_complex.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, fp, fp, C.c_int, vp]
     lib.tetra_dos_select.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, ip, C.c_int, C.c_int, fp, fp, C.c_int, vp]
+    lib.tetra_eigh.argtypes = [vp, fp, fp, fp, vp]
     lib.tetra_weights.argtypes = [vp, fp, C.c_int, fp, C.c_int, fp, fp, vp]
     lib.tetra_dos_partial.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, C.c_int, C.c_int, vp, vp]
     lib.tetra_dos_finalize.argtypes = [vp, vp, C.c_int, fp, fp, vp]
@@ -141,6 +142,10 @@ class Plan:
         _check(load().tetra_dos_select(self._h, _ptr(E), _ptr(W), layout, _ptr(omega), nE, orb, len(orbitals),
                                        1 if want_total else 0, _ptr(dos), _ptr(nos), memspace,
                                        _stream_ptr(stream, memspace)), "tetra_dos_select")
+
+    def tetra_eigh(self, H, E, A, stream=None):
+        """tetra_eigh(): device tensors H[nk][nb][nb] complex64 (or float pairs) -> E[nk][nb], A[nk][nb][nb] complex64."""
+        _check(load().tetra_eigh(self._h, _ptr(H), _ptr(E), _ptr(A), _stream_ptr(stream, TDOS_DEVICE)), "tetra_eigh")
 
     def tetra_weights(self, E, energies, wk, dwk=None, layout: int = TDOS_AOS, stream=None):
         """tetra_weights(): per-k-point integration weights wk[nW][nb][nk] (and dwk) for device tensors."""

@@ -9,7 +9,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libtetrados.so")
 SOURCES = [os.path.join(CSRC, "tetrados.cu")]
 HEADERS = [os.path.join(CSRC, "tdos_kernels.cuh"), os.path.join(CSRC, "tdos_weights.cuh"),
-           os.path.join(CSRC, "tdos_main5.cuh"), os.path.join(CSRC, "tdos_kweights.cuh"),
+           os.path.join(CSRC, "tdos_main5.cuh"), os.path.join(CSRC, "tdos_kweights.cuh"), os.path.join(CSRC, "tdos_eigh.cuh"),
            os.path.join(os.path.dirname(_HERE), "include", "tetrados.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

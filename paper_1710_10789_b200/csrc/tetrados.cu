@@ -12,6 +12,7 @@
 #include <new>
 #include <vector>
 
+#include "tdos_eigh.cuh"
 #include "tdos_kernels.cuh"
 #include "tdos_kweights.cuh"
 #include "tdos_main5.cuh"
@@ -704,6 +705,23 @@ int tetra_weights(tdos_plan* p, const float* E, int layout, const float* energie
     long long blocks = (total + 255) / 256;
     if (blocks > (long long)p->num_sms * 32) blocks = (long long)p->num_sms * 32;
     tdos::tdos_kweights<<<(int)blocks, 256, 0, st>>>(kp);
+    CK(cudaGetLastError());
+    return TDOS_OK;
+}
+
+int tetra_eigh(tdos_plan* p, const float* H, float* E, float* A, void* cuda_stream) {
+    if (!p || !H || !E || !A) return TDOS_EINVAL;
+    if (p->nb != p->norb || p->nb > 8) return TDOS_EINVAL;   // square problems of order <= 8 (the paper's model: 8)
+    ON_DEVICE(p->device);
+    tdos::EighParams ep{};
+    ep.H = reinterpret_cast<const float2*>(H);
+    ep.E = E;
+    ep.A = reinterpret_cast<float2*>(A);
+    ep.nmat = (long long)p->nk[0] * p->nk[1] * p->nk[2];
+    ep.nb = p->nb;
+    ep.sweeps = 10;
+    const long long threads = ep.nmat * 8;
+    tdos::tdos_eigh8<<<(unsigned)((threads + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(ep);
     CK(cudaGetLastError());
     return TDOS_OK;
 }

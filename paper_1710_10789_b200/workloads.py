@@ -152,6 +152,24 @@ def _tb8_chunk(p: dict, k: np.ndarray):
     return w.astype(np.float32), np.ascontiguousarray(Wt.transpose(0, 2, 1)).astype(np.float32)
 
 
+def tb8_hamiltonian(nk, chunk: int = 65536) -> np.ndarray:
+    """The normalised Hamiltonian itself, H[ik][8][8] complex64 (exactly Hermitian after the cast): the input of the
+    device-side eigensolver (Eq. 1).  tb8_bands diagonalises the same matrices on the host in complex128."""
+    p = load_tb8_params()
+    lo, hi = p["norm_lo"], p["norm_hi"]
+    c, s = 0.5 * (lo + hi), 8.0 / (hi - lo)
+    k = kgrid(nk)
+    out = np.empty((k.shape[0], 8, 8), dtype=np.complex64)
+    for s0 in range(0, k.shape[0], chunk):
+        H = _tb8_hraw(p, k[s0:s0 + chunk])
+        H -= c * np.eye(8)
+        H *= s
+        H -= np.eye(8)
+        H = 0.5 * (H + H.conj().transpose(0, 2, 1))
+        out[s0:s0 + chunk] = H.astype(np.complex64)
+    return out
+
+
 def tb8_bands(nk, threads: int | None = None, chunk: int = 16384):
     """Configs 2-5: E[ik][8] ascending (fp32), W[ik][n][m] = |U[m][n]|^2 (fp32).
     H(k) = s*(H_raw(k) - c) - 1 with c, s from the Nk=16 spectrum so that the

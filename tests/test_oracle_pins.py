@@ -466,3 +466,27 @@ def test_per_k_weights_reproduce_the_orbital_sums(oracle_lib):
         assert not wk[0].any() and not dwk[0].any()
         assert np.allclose(wk[-1], 1.0 / np.prod(nk), rtol=1e-13) and not dwk[-1].any()
         assert (wk >= 0).all()
+
+
+def test_eigh_bands_pins(oracle_lib):
+    """Pin of oracle.eigh_bands (Eq. 1): a closed-form 2 x 2 Hermitian matrix [[a, g], [conj(g), b]] has
+    E = (a+b)/2 -+ sqrt(((a-b)/2)^2 + |g|^2) and |a_-^1|^2 = (1 + (b-a)/(2 r)) / 2 with r the square root; for the
+    seeded 8-orbital Hamiltonian H a = E a holds to rounding, the weights of every band and of every orbital sum to 1,
+    and the result equals what workloads.tb8_bands (an independent call path) delivers."""
+    a, b, g = 0.3, -1.1, 0.4 - 0.7j
+    H = np.array([[[a, g], [np.conj(g), b]]])
+    E, W = oracle_lib.eigh_bands(H)
+    r = np.sqrt(((a - b) / 2) ** 2 + abs(g) ** 2)
+    assert np.allclose(E[0], [(a + b) / 2 - r, (a + b) / 2 + r], rtol=1e-14)
+    w_lower_on_orbital0 = 0.5 * (1 + (b - a) / (2 * r))
+    assert np.allclose(W[0, 0], [w_lower_on_orbital0, 1 - w_lower_on_orbital0], rtol=1e-13)
+    nk = (4, 3, 5)
+    H = wl.tb8_hamiltonian(nk)
+    assert np.array_equal(H, H.conj().transpose(0, 2, 1))                      # exactly Hermitian after the cast
+    E, W = oracle_lib.eigh_bands(H)
+    assert np.all(np.diff(E, axis=1) >= 0)
+    assert np.allclose(W.sum(axis=1), 1.0, atol=1e-13) and np.allclose(W.sum(axis=2), 1.0, atol=1e-13)
+    w, U = np.linalg.eigh(H.astype(np.complex128))
+    assert np.abs(np.einsum("kij,kjn->kin", H.astype(np.complex128), U) - U * w[:, None, :]).max() < 1e-13
+    Eb, Wb = wl.tb8_bands(nk, threads=1)
+    assert np.abs(E - Eb).max() < 2e-6 and np.abs(W - Wb).max() < 2e-5      # complex64 H against complex128 H
