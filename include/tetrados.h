@@ -22,19 +22,31 @@
  *   normalisation   V_T/V_G = 1/(6 N1 N2 N3); no spin factor.  N_m(w -> inf) = (1/nk) sum_k sum_n b.
  *   intervals       half-open, tested in the order  w <= E1, w < E2, w < E3, w < E4, else  (reading G10).
  *   precision       fp32 inputs, fp32 arithmetic for the weights, block-local fp32
- *                   partial sums, fp64 merge across blocks and fp64 prefix sum for N; fp32 outputs.
+ *                   partial sums, fp64 merge across blocks and fp64 prefix sum for N; fp32 outputs
+ *                   (tdos_plan_set_accumulation widens every sum to fp64).
+ *   reproducibility results are reproducible to rounding, NOT bit for bit: the block partials are built with
+ *                   fire-and-forget reductions in L2 (red.global.add) in arrival order and work items are drawn
+ *                   from a global counter, so the order of the fp32 additions differs from run to run
+ *                   (differences ~1e-7 relative, two orders below the tolerances of BASELINE.json).
  *   NaN/Inf in E or W are not detected: results are then undefined.
+ *   omega           must be strictly increasing.  Host mode checks it (TDOS_EINVAL); DEVICE mode does NOT -- the
+ *                   array lives on the device and the call only enqueues work -- a non-monotonic device array
+ *                   gives undefined results (no fault: bin indices are clamped to [0, nE]).
  *
- * Kernels: tdos_main5 (one record per interval of Eq. 12-14; norb >= 5 and norb % 4 == 0) or tdos_main (any norb);
- * the environment variables TDOS_KERNEL=3|5 and TDOS_TILE=<index>, read at plan creation, override the choice of
- * kernel and tile shape for experiments.  Without TDOS_KERNEL a plan that started with
- * tdos_main5 reads the work counters of its first call when the second call starts (one host-side wait for the
- * first call's kernel) and keeps tdos_main from then on if the windows average fewer than 6 energies.
+ * Kernels: tdos_main5 (one record per interval of Eq. 12-14; blocks of 8 orbitals: norb >= 5 and norb % 4 == 0) and
+ * tdos_main (one record per tetrahedron; any norb).  A plan that qualifies for tdos_main5 carries both: every call
+ * first enqueues tdos_estimate, which samples the windows (E1, E4) of 2048 cubes on the device, then both main
+ * kernels; the one that suits the windows runs (tdos_main below 6 energies per window on average, tdos_main5
+ * above), the other returns at once.  Nothing is decided on the host and nothing is remembered between calls.
+ * Environment variables read at plan creation, for experiments only: TDOS_KERNEL=3|5 forces one kernel, TDOS_TILE=<index>
+ * picks another compiled tile shape, TDOS_BLOCKS_PER_SM=<n> lowers the number of resident blocks.
  *
  * Ownership: the caller owns every array; the library never frees them and does not retain them
  * past the call (device mode: past completion of the work queued on `stream`).  A plan owns all
- * scratch (block partials, staging buffers, its side stream).  A plan must not be used from two
- * host threads or two streams at the same time.  Inputs are never written.
+ * scratch (block partials, staging buffers, its side stream), shared by all its calls: calls are executed one after the
+ * other even when issued on different streams (a call on another stream than the previous one first waits, on the
+ * device, for that one's end).  A plan must not be used from two host threads at the same time.  Inputs are never
+ * written.  Every entry point runs on the plan's device and restores the caller's current device before it returns.
  *
  * Errors: every function returns 0 (TDOS_OK) or a negative code; nothing throws, exits or prints.
  * On error the outputs are untouched (host mode) / unspecified only if TDOS_ECUDA occurred mid-flight.
@@ -77,8 +89,8 @@ const char* tdos_last_cuda_error(void);
 /*
  * Create a plan for grids of nk[0] x nk[1] x nk[2] k-points, nb bands, norb orbitals and up to
  * nE_max energies on CUDA device `device`.  Allocates all device scratch:
- * per-block partial histograms (3 * norb * nE_max floats per resident block) and the fp64 merge
- * buffers.  *out is set only on success.
+ * per-block partial histograms (3 * (norb + 1 rounded up to 4) * (nE_max + 3) floats per resident block, 148 blocks on
+ * a B200) and the fp64 merge buffer.  *out is set only on success.
  */
 int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int norb, int nE_max);
 
@@ -109,7 +121,7 @@ int tdos_plan_destroy(tdos_plan* p);
  *  dos     out [norb][nE], overwritten
  *  nos     out [norb][nE], overwritten; may be NULL
  *  memspace TDOS_DEVICE: all five pointers are device pointers; the call only enqueues work on
- *          `cuda_stream` (a cudaStream_t, NULL = legacy default stream) and returns.
+ *          `cuda_stream` (a cudaStream_t, NULL = legacy default stream) and returns; no host synchronisation.
  *          TDOS_HOST: all five are host pointers; inputs are staged to the device in z-slabs on the
  *          plan's side stream, overlapped with the kernels, and the call returns after the results
  *          are in `dos` / `nos` (`cuda_stream` is ignored).
@@ -197,11 +209,13 @@ int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, f
  *   the main kernel: cnt[0] = n_tb = (tetrahedron, band) pairs processed, cnt[1] = n_eval = number of
  *   (tetrahedron, band, omega_i) with E1 < omega_i < E4, i.e. evaluations of Eq. 12-14 the method
  *   needs; cnt[2] = how many of them fall in the middle interval E2 <= omega_i < E3
- *   (Eq. 13; -1 if the kernel generation does not count it), cnt[3] = main kernel generation (3 or 4).
+ *   (Eq. 13; -1 if the kernel that ran does not count it), cnt[3] = generation of the main kernel that ran
+ *   (3 = tdos_main, 5 = tdos_main5; for a plan carrying both: what the device decided for that call).
  *   Synchronises the call's stream.
  * tdos_kernel_ms: mean device time of the main kernel and of the merge+finalize kernels over the
  *   last `ncalls` (1..64) device-mode tetra_dos calls on this plan, from CUDA events the library records
- *   on each call's stream around its own launches (waits for those calls to finish).
+ *   on each call's stream around its own launches (waits for those calls to finish); the "main kernel" bracket
+ *   holds the scratch memsets, tdos_estimate and both main kernels of a plan that carries two.
  *   tdos_last_kernel_ms is tdos_kernel_ms with ncalls = 1.
  * tdos_fp32_fma_probe: runs a register-resident FFMA chain on every SM of the plan's device and
  *   returns the achieved FP32 rate in TFLOP/s (2 flops per FMA lane) in *tflops.

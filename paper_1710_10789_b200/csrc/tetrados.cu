@@ -628,10 +628,19 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
         for (int i = 2; i >= 0; i--) sizes[ns++] = (double)(kFirstSlabBytes << i);
         zb[0] = 0;
         double acc = 0.0;
+        // every slab is tiled from its own first plane, so a slab whose length is not a multiple of the tile's extent
+        // in z ends in a layer of partly empty tiles: lengths are rounded to whole tiles (the short first slab, which
+        // only has to start the kernels early, and the remainder at the end excepted)
+        const int tz = p->var.TZ;
         for (int i = 0; i < ns && zb[nslab] < N3; i++) {
             acc += sizes[i] * scale;
             int z = (int)(acc / plane_bytes + 0.5);
             if (z <= zb[nslab]) z = zb[nslab] + 1;
+            if (i > 0 && tz > 1) {
+                int len = ((z - zb[nslab] + tz / 2) / tz) * tz;
+                if (len < tz) len = tz;
+                z = zb[nslab] + len;
+            }
             if (z > N3 || i == ns - 1) z = N3;
             zb[++nslab] = z;
         }
