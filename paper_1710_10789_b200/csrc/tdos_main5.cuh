@@ -44,6 +44,41 @@ __device__ __forceinline__ int locate5(const float* om, int nE, float om0, float
     return i;
 }
 
+// The four bins of a (tetrahedron, band) at once: i1 = first omega > e0, i2, i3, i4 = first omega >= e1, e2, e3.
+// All index guesses and the eight energies next to them are fetched before any of them is looked at, so the loads
+// overlap; the exact fix-up loops of locate5 only run where a guess is off by more than its own bin.
+__device__ __forceinline__ void locate5x4(const float* om, int nE, float om0, float inv_dom, float e0, float e1, float e2,
+                                          float e3, int& i1, int& i2, int& i3, int& i4) {
+    const float x[4] = {e0, e1, e2, e3};
+    int g[4];
+    float a[4], b[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        float gq = (x[k] - om0) * inv_dom;
+        gq = fminf(fmaxf(gq, 0.0f), (float)nE);
+        g[k] = (int)gq;
+        a[k] = om[max(g[k] - 1, 0)];
+        b[k] = om[min(g[k], nE - 1)];
+    }
+    int r[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        int i = g[k];
+        if (k == 0) {   // strict: first omega > x
+            if (i > 0 && a[k] > x[k]) { --i; while (i > 0 && om[i - 1] > x[k]) --i; }
+            else if (i < nE && b[k] <= x[k]) { ++i; while (i < nE && om[i] <= x[k]) ++i; }
+        } else {        // first omega >= x
+            if (i > 0 && a[k] >= x[k]) { --i; while (i > 0 && om[i - 1] >= x[k]) --i; }
+            else if (i < nE && b[k] < x[k]) { ++i; while (i < nE && om[i] < x[k]) ++i; }
+        }
+        r[k] = i;
+    }
+    i1 = r[0];
+    i2 = max(i1, r[1]);
+    i3 = max(i2, r[2]);
+    i4 = max(i3, r[3]);
+}
+
 template <int TX, int TY, int TZ>
 struct Cfg5 {
     static constexpr int MB = 8;
@@ -523,10 +558,8 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
                 uint32_t rl = 0, rh = 0, rm = 0;               // empty ranges
                 if (valid) {
                     // bins (reading G10): low [i1,i2), mid [i2,i3), high [i3,i4), full weight from i4 on
-                    const int i1 = locate5<true>(om_loc, nE, om0, inv_dom, e0);             // first omega > E1
-                    const int i2 = max(i1, locate5<false>(om_loc, nE, om0, inv_dom, e1));   // first omega >= E2
-                    const int i3 = max(i2, locate5<false>(om_loc, nE, om0, inv_dom, e2));
-                    const int i4 = max(i3, locate5<false>(om_loc, nE, om0, inv_dom, e3));
+                    int i1, i2, i3, i4;   // first omega > E1; first omega >= E2, E3, E4
+                    locate5x4(om_loc, nE, om0, inv_dom, e0, e1, e2, e3, i1, i2, i3, i4);
                     rl = (uint32_t)i1 | ((uint32_t)i2 << 16);
                     rm = (uint32_t)i2 | ((uint32_t)i3 << 16);
                     rh = (uint32_t)i3 | ((uint32_t)i4 << 16);
