@@ -110,6 +110,22 @@ __device__ __forceinline__ int locate_bin(const float* __restrict__ omega, int n
     return i;
 }
 
+// i1 = first omega > e_lo, i4 = first omega >= e_hi (or i1 if the two energies coincide) on an energy array in any
+// address space: both index guesses and the four energies next to them are fetched before any is looked at, so the
+// loads overlap; the exact fix-up loops only run where a guess is off by more than its own bin.
+__device__ __forceinline__ void locate_window(const float* om, int nE, float om0, float inv_dom, float e_lo, float e_hi,
+                                              int& i1, int& i4) {
+    float g1 = fminf(fmaxf((e_lo - om0) * inv_dom, 0.0f), (float)nE), g4 = fminf(fmaxf((e_hi - om0) * inv_dom, 0.0f), (float)nE);
+    int a = (int)g1, b = (int)g4;
+    const float a0 = om[max(a - 1, 0)], a1 = om[min(a, nE - 1)], b0 = om[max(b - 1, 0)], b1 = om[min(b, nE - 1)];
+    if (a > 0 && a0 > e_lo) { --a; while (a > 0 && om[a - 1] > e_lo) --a; }
+    else if (a < nE && a1 <= e_lo) { ++a; while (a < nE && om[a] <= e_lo) ++a; }
+    if (b > 0 && b0 >= e_hi) { --b; while (b > 0 && om[b - 1] >= e_hi) --b; }
+    else if (b < nE && b1 < e_hi) { ++b; while (b < nE && om[b] < e_hi) ++b; }
+    i1 = a;
+    i4 = (e_hi > e_lo) ? b : a;
+}
+
 #define TDOS_CSWAP(ea, eb, ca, cb)            \
     do {                                      \
         if (eb < ea) {                        \
@@ -322,6 +338,14 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     const int nE = p.nE;
     const int norb = p.norb;
     const float* __restrict__ omega = p.omega;
+    // the energy grid is probed 4 times per (tetrahedron, band): keep a block-wide copy in shared memory when it fits
+    const float* om_loc = omega;
+    if (p.om_smem) {
+        float* sOmAll = reinterpret_cast<float*>(smem + (size_t)NWARP * Cfg::bytes);
+        for (int i = threadIdx.x; i < nE; i += NWARP * 32) sOmAll[i] = __ldg(omega + i);
+        __syncthreads();
+        om_loc = sOmAll;
+    }
     const float om0 = __ldg(omega);
     float inv_dom = 0.0f;
     if (nE > 1) {
@@ -421,9 +445,8 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 TDOS_CSWAP(e1, e2, c1, c2);
                 c0 *= WST; c1 *= WST; c2 *= WST; c3 *= WST;   // float offsets into sW
                 if (valid) {
-                    const int i1 = locate_bin<true>(omega, nE, om0, inv_dom, e0);      // first omega > E1
-                    // first omega >= E4, and > E1 (test order G10)
-                    const int i4 = (e3 > e0) ? locate_bin<false>(omega, nE, om0, inv_dom, e3) : i1;
+                    int i1, i4;   // first omega > E1; first omega >= E4, and > E1 (test order G10)
+                    locate_window(om_loc, nE, om0, inv_dom, e0, e3, i1, i4);
                     rng = (uint32_t)i1 | ((uint32_t)i4 << 16);
                     if (mb == 0) {   // work counters (exact integers; bench.py's flop count uses them)
                         cnt_tb += 1;

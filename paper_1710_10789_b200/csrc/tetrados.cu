@@ -428,10 +428,10 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         if (items > 0x7fffffffLL) return TDOS_EINVAL;
         mp.n_items = (int)items;
         if (!which) items_main = items;
-        // generation 5: a block-wide copy of omega in shared memory if the device limit allows it
+        // a block-wide copy of omega in shared memory if the device limit allows it
         size_t smem = v.smem;
         mp.om_smem = 0;
-        if (v.gen == 5 && v.smem + (size_t)nE * sizeof(float) <= p->smem_optin) {
+        if (v.smem + (size_t)nE * sizeof(float) <= p->smem_optin) {
             mp.om_smem = 1;
             smem += (size_t)nE * sizeof(float);
         }
