@@ -573,3 +573,19 @@ def test_fp64_accumulation_on_unstructured_energies(nk, nb, norb, nE):
             want = {"dos": np.concatenate([ref["dos"][[2, 0]], ref["dos"].sum(axis=0, keepdims=True)]),
                     "nos": np.concatenate([ref["nos"][[2, 0]], ref["nos"].sum(axis=0, keepdims=True)])}
             assert_parity(want, ddos.cpu().numpy(), dnos.cpu().numpy(), "fp64 select")
+
+
+@pytest.mark.parametrize("kernel", ["3", "5"])
+def test_many_energies_no_shared_memory_copy_of_omega(kernel, monkeypatch):
+    """30 000 energies: the block-wide copy of omega no longer fits beside the warps' slices (the kernels read the
+    global array), windows span hundreds of bins and many 128-bin passes; norb = 16 (two orbital blocks)."""
+    monkeypatch.setenv("TDOS_KERNEL", kernel)
+    nk, nb, norb, nE = (6, 5, 4), 2, 16, 30000
+    E, W = wl.random_bands(nk, nb, norb, seed=77)
+    om = wl.omega_grid(-1.2, 1.3, nE)
+    ref = oracle.tetra_dos(E, W, nk, om, windowed=True)
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        dos, nos = run_gpu(E, W, nk, om, plan=plan)
+        cnt = plan.last_counters()
+    assert cnt["kernel"] == int(kernel) and cnt["n_eval"] == ref["n_eval"]
+    assert_parity(ref, dos, nos, "30000 energies, kernel " + kernel)
