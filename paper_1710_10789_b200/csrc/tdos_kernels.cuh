@@ -63,8 +63,10 @@ struct MainParams {
 };
 
 // Mean number of bins with E1 < omega < E4 per (tetrahedron, band) below which tdos_main (generation 3: one record per
-// tetrahedron) beats tdos_main5 (generation 5: one record per interval of Eq. 12-14) -- config 5's windows are 3 bins.
-constexpr unsigned long long kShortWindowBins = 6;
+// tetrahedron, groups of one lane = chunks of 2 bins) beats tdos_main5 (generation 5: one record per interval of
+// Eq. 12-14, chunks of 4 bins) -- config 5's windows are 3 bins.  Measured on the Nk = 64 grid: 6.6 bins 1.20 against
+// 1.24 ms, 8.4 bins 1.42 against 1.37 ms.
+constexpr unsigned long long kShortWindowBins = 7;
 __host__ __device__ __forceinline__ int wanted_generation(unsigned long long sum_bins, unsigned long long n_tb) {
     return (n_tb > 0 && sum_bins < kShortWindowBins * n_tb) ? 3 : 5;
 }
@@ -320,7 +322,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
     constexpr int CH = 2 * GL;              // bins per chunk: every lane owns two adjacent bins
     constexpr int PASS = NCH * CH;          // bins per pass
     constexpr unsigned FULL = 0xffffffffu;
-    static_assert(GL == 2 || GL == 4 || GL == 8 || GL == 16, "group width");
+    static_assert(GL == 1 || GL == 2 || GL == 4 || GL == 8 || GL == 16, "group width");
 
     extern __shared__ __align__(16) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;

@@ -113,8 +113,11 @@ int pick_mb(int norb) { return norb <= 1 ? 1 : norb <= 2 ? 2 : norb <= 4 ? 4 : 8
 template <int MB>
 std::vector<Variant> variants_for() {
     return {make_variant<MB, 4, 4, 2, 2, 16>(), make_variant<MB, 4, 4, 2, 4, 16>(), make_variant<MB, 4, 4, 4, 2, 12>(),
-            make_variant<MB, 4, 4, 4, 4, 12>(), make_variant<MB, 4, 4, 2, 2, 20>()};
+            make_variant<MB, 4, 4, 4, 4, 12>(), make_variant<MB, 4, 4, 2, 2, 20>(),
+            // groups of ONE lane (chunks of 2 bins): the short-window kernel of plans that carry two
+            make_variant<MB, 4, 4, 2, 1, 16>(), make_variant<MB, 2, 2, 8, 1, 16>()};
 }
+constexpr int kShortVariant = 5, kShortVariantZ8 = 6;   // indices into variants_for<8>()
 
 std::vector<Variant> variants(int MB) {
     switch (MB) {
@@ -291,7 +294,8 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     // 3 bins on average) are served better by one record per tetrahedron (generation 3) than by three (generation 5).
     // Which one runs is decided per call on the device, from a sample of the windows (tdos_estimate).
     if (gen == 5 && !kv) {
-        p->var_short = variants(8)[0];
+        // one record per tetrahedron, chunks of 2 bins; long in z like the main kernel's tile when the grid divides
+        p->var_short = variants(8)[(nk[2] % 8 == 0 && nk[0] % 2 == 0 && nk[1] % 2 == 0) ? kShortVariantZ8 : kShortVariant];
         int bps = 0;
         if (setup(p->var_short, &bps) == cudaSuccess && bps >= 1) {
             p->adaptive = true;

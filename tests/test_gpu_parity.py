@@ -61,18 +61,21 @@ def test_random_small_grids(nk, nb, norb, nE):
     assert_parity(ref, dos, None, "random %s nos=NULL" % (nk,))
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
-def test_every_compiled_kernel_configuration(variant, monkeypatch):
-    """TDOS_TILE selects the tile shape / group width / warps per block compiled into the library;
-    every one of them must reproduce the oracle (tb8 model: several tiles + ragged tails; random
-    energies: windows spanning many passes)."""
+@pytest.mark.parametrize("kernel,variant", [("5", v) for v in range(5)] + [("3", v) for v in range(7)])
+def test_every_compiled_kernel_configuration(kernel, variant, monkeypatch):
+    """TDOS_KERNEL / TDOS_TILE select the kernel and the tile shape / group width / warps per block compiled into the
+    library; every one of them must reproduce the oracle (tb8 model: several tiles + ragged tails; random energies,
+    3 orbitals -- always tdos_main: windows spanning many passes)."""
+    monkeypatch.setenv("TDOS_KERNEL", kernel)
     monkeypatch.setenv("TDOS_TILE", str(variant))
     nk = (10, 9, 7)
     E, W = wl.tb8_bands(nk, threads=1)
     om = wl.omega_grid(-6.0, 4.0, 777)
     ref = oracle.tetra_dos(E, W, nk, om, nthreads=_threads())
-    dos, nos = run_gpu(E, W, nk, om)
-    assert_parity(ref, dos, nos, "tb8 variant %d" % variant)
+    with binding.Plan(nk, 8, 8, 777) as plan:
+        dos, nos = run_gpu(E, W, nk, om, plan=plan)
+        assert plan.last_counters()["kernel"] == int(kernel)
+    assert_parity(ref, dos, nos, "tb8 kernel %s variant %d" % (kernel, variant))
     nk = (5, 6, 4)
     E, W = wl.random_bands(nk, 2, 3, seed=9)
     om = wl.omega_grid(-1.1, 1.1, 1500)
