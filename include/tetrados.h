@@ -36,7 +36,7 @@
  * Kernels: tdos_main5 (one record per interval of Eq. 12-14; blocks of 8 orbitals: norb >= 5 and norb % 4 == 0) and
  * tdos_main (one record per tetrahedron; any norb).  A plan that qualifies for tdos_main5 carries both: every call
  * first enqueues tdos_estimate, which samples the windows (E1, E4) of 2048 cubes on the device, then both main
- * kernels; the one that suits the windows runs (tdos_main below 6 energies per window on average, tdos_main5
+ * kernels; the one that suits the windows runs (tdos_main below 7 energies per window on average, tdos_main5
  * above), the other returns at once.  Nothing is decided on the host and nothing is remembered between calls.
  * Environment variables read at plan creation, for experiments only: TDOS_KERNEL=3|5 forces one kernel, TDOS_TILE=<index>
  * picks another compiled tile shape, TDOS_BLOCKS_PER_SM=<n> lowers the number of resident blocks.
