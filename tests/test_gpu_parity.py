@@ -398,7 +398,7 @@ def test_per_k_integration_weights(nk, nb):
 
 def test_plan_picks_kernel_per_call_on_the_device(monkeypatch):
     """Unless TDOS_KERNEL is set, a plan on 8 orbitals enqueues both main kernels and a sample of the windows, taken on
-    the device at the start of every call, decides which one runs: tdos_main (one record per tetrahedron) below 6 bins
+    the device at the start of every call, decides which one runs: tdos_main (one record per tetrahedron) below 7 bins
     per window, tdos_main5 above.  The same plan serves a coarse and a fine energy grid in turn; every call is checked."""
     monkeypatch.delenv("TDOS_KERNEL", raising=False)
     nk, nb, norb = (8, 8, 8), 2, 8
