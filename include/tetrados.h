@@ -65,6 +65,8 @@ extern "C" {
 #define TDOS_ENOMEM  -2   /* host or device allocation failed                                          */
 #define TDOS_ECUDA   -3   /* a CUDA call failed; see tdos_last_cuda_error()                            */
 #define TDOS_EARCH   -4   /* the selected device is not compute capability 10.x (sm_100)               */
+#define TDOS_ESIZE   -5   /* tetra_dos_static only: the problem needs more scratch than the library's built-in
+                             buffer holds (norb * nE above TDOS_STATIC_MAX_CELLS); use a plan instead  */
 
 #define TDOS_AOS 0        /* E[ik][n],  W[ik][n][m]   -- what a CPU code usually holds                  */
 #define TDOS_SOA 1        /* E[n][ik],  W[n][m][ik]   -- k fastest                                      */
@@ -198,6 +200,50 @@ int tetra_weights(tdos_plan* p, const float* E, int layout, const float* energie
  */
 int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, float omega_min,
                      float omega_max, int nE, float* dos, float* nos);
+
+/*
+ * tetra_dos for callers that are not allowed to allocate device memory.
+ *
+ * Who that is: code that runs where cudaMalloc is off limits -- a plug-in inside a host program (a DFT/DMFT driver,
+ * say) that has sized its own memory pools to fill the GPU and requires every byte of device memory to come from
+ * them, so a cudaMalloc either fails or breaks the host's accounting; and a self-consistency or real-time loop that
+ * cannot afford the device-wide synchronisation that cudaMalloc / cudaFree imply in the middle of its pipeline.
+ * A tdos_plan is no use to them: creating one allocates its block partials, merge buffer, streams and events.
+ *
+ * This call needs no plan and allocates nothing -- no cudaMalloc, no cudaFree, no stream, no event.  The scratch every
+ * DOS call needs (block-partial histograms, the fp64 merge buffer, the work counters) lives in an array that is built
+ * into the library image: TDOS_STATIC_SCRATCH_BYTES (about 16.8 MB) of device memory on EVERY GPU on which the
+ * process loads the library, held until the process exits whether or not this function is ever called.  The price
+ * of a fixed buffer is a size limit:
+ *
+ *     norb * (nE rounded up to a multiple of 4)  <=  TDOS_STATIC_MAX_CELLS  (32768: e.g. 8 orbitals x 4096 energies,
+ *                                                                            16 x 2048, 1 x 32768)
+ *
+ * Anything larger returns TDOS_ESIZE and touches nothing.  The fewer cells a call uses, the more thread blocks get a
+ * private histogram (up to one per resident block; at the limit 42 blocks share the GPU), so small problems run at
+ * plan speed and problems at the limit run slower than through a plan.
+ *
+ * Arguments as tetra_dos in TDOS_DEVICE mode: E, W (NULL = unit weights, needs norb == 1), omega, dos, nos (may be
+ * NULL) are device pointers on the CURRENT device, which must be an sm_100 GPU (TDOS_EARCH otherwise); the grid shape,
+ * nb and norb are passed directly since there is no plan; the work is enqueued on `cuda_stream` and the call returns
+ * without waiting.  Only the one-record-per-tetrahedron kernel (tdos_main) is used; results agree with tetra_dos to
+ * rounding (different summation order), not bit for bit.
+ *
+ * First call on a device: looks up the device address of the built-in buffer, sets the kernels' shared-memory limit
+ * and queries their occupancy, and remembers all three for later calls (guarded by a mutex; later calls only check a
+ * flag).  Make that first call per device outside any stream capture; it is also the call that may trigger the CUDA
+ * runtime's own lazy loading of the kernels.
+ *
+ * All calls in a process share the one buffer per device.  Each call clears what it needs before it uses it, so
+ * calls that follow each other on one stream (or are otherwise ordered on the GPU) are independent of each other's
+ * sizes and contents.  Calls that can OVERLAP on the same GPU -- two streams, two host threads -- race on the buffer
+ * and give wrong results without any error; ordering them is the caller's job.  Plans are unaffected: they use their
+ * own scratch.
+ */
+#define TDOS_STATIC_MAX_CELLS     32768
+#define TDOS_STATIC_SCRATCH_BYTES (256 + 3 * TDOS_STATIC_MAX_CELLS * 8 + (16 << 20))
+int tetra_dos_static(const int nk[3], int nb, int norb, const float* E, const float* W, int layout,
+                     const float* omega, int nE, float* dos, float* nos, void* cuda_stream);
 
 /*
  * Diagnostics used by bench.py (not part of the hot path).

@@ -10,15 +10,16 @@ import os
 
 from . import build as _build
 
-TDOS_OK, TDOS_EINVAL, TDOS_ENOMEM, TDOS_ECUDA, TDOS_EARCH = 0, -1, -2, -3, -4
+TDOS_OK, TDOS_EINVAL, TDOS_ENOMEM, TDOS_ECUDA, TDOS_EARCH, TDOS_ESIZE = 0, -1, -2, -3, -4, -5
 TDOS_AOS, TDOS_SOA = 0, 1
 TDOS_ACC_FP32, TDOS_ACC_FP64 = 0, 1
 TDOS_DEVICE, TDOS_HOST = 0, 1
 TDOS_MAX_NE = 65534
+TDOS_STATIC_MAX_CELLS = 32768   # tetra_dos_static: norb * (nE rounded up to 4) it accepts
 
 # every symbol include/tetrados.h declares
 SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy", "tdos_plan_set_accumulation",
-           "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_eigh", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tdos_plan_info",
+           "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_eigh", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tetra_dos_static", "tdos_plan_info",
            "tdos_last_counters", "tdos_kernel_ms", "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
 
 _lib = None
@@ -59,6 +60,7 @@ def load():
     lib.tetra_dos_partial.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, C.c_int, C.c_int, vp, vp]
     lib.tetra_dos_finalize.argtypes = [vp, vp, C.c_int, fp, fp, vp]
     lib.tetra_dos_simple.argtypes = [fp, fp, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_int, fp, fp]
+    lib.tetra_dos_static.argtypes = [ip, C.c_int, C.c_int, fp, fp, C.c_int, fp, C.c_int, fp, fp, vp]
     lib.tdos_plan_info.argtypes = [vp, C.POINTER(C.c_longlong)]
     lib.tdos_last_counters.argtypes = [vp, C.POINTER(C.c_longlong)]
     lib.tdos_kernel_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float)]
@@ -200,6 +202,18 @@ def tetra_dos_simple(E, W, Nk: int, nb: int, norb: int, omega_min: float, omega_
     """tetra_dos_simple(): host arrays, AoS, cubic grid, uniform omega; one-shot."""
     _check(load().tetra_dos_simple(_ptr(E), _ptr(W), int(Nk), int(nb), int(norb), float(omega_min), float(omega_max),
                                    int(nE), _ptr(dos), _ptr(nos)), "tetra_dos_simple")
+
+
+def tetra_dos_static(nk, nb: int, norb: int, E, W, omega, dos, nos=None, layout: int = TDOS_AOS, stream=None):
+    """tetra_dos_static(): tetra_dos on device tensors without a plan and without a single device allocation, for
+    callers that are barred from cudaMalloc (a plug-in in a host code that owns all GPU memory through its own pools, a
+    loop that cannot take cudaMalloc's device-wide synchronisation).  The scratch is a fixed buffer inside the library,
+    so norb * (nE rounded up to 4) must not exceed TDOS_STATIC_MAX_CELLS (TdosError with code TDOS_ESIZE otherwise),
+    and calls that could overlap on one GPU must be ordered by the caller: they all share that buffer.  Runs on the
+    current device; the first call per device also does the one-time set-up (include/tetrados.h)."""
+    arr = (C.c_int * 3)(*[int(x) for x in nk])
+    _check(load().tetra_dos_static(arr, int(nb), int(norb), _ptr(E), _ptr(W), layout, _ptr(omega), int(omega.shape[0]),
+                                   _ptr(dos), _ptr(nos), _stream_ptr(stream, TDOS_DEVICE)), "tetra_dos_static")
 
 
 def tdos_version() -> int:

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -201,6 +202,7 @@ const char* tdos_strerror(int code) {
         case TDOS_ENOMEM: return "out of memory";
         case TDOS_ECUDA: return "CUDA error (see tdos_last_cuda_error)";
         case TDOS_EARCH: return "device is not compute capability 10.x (sm_100)";
+        case TDOS_ESIZE: return "problem exceeds the built-in scratch of tetra_dos_static (norb * nE > TDOS_STATIC_MAX_CELLS)";
         default: return "unknown error code";
     }
 }
@@ -864,3 +866,158 @@ int tdos_fp32_fma_probe(tdos_plan* p, int packed, double* tflops) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// tetra_dos_static: the path for callers that must not allocate (include/tetrados.h).  All scratch of one call sits in
+// this array, which is part of the library image: the driver places a copy on every GPU that loads the library and
+// keeps it until the process ends.  Layout (bytes):
+//     [0, 64)                          work counters of tdos_main (8 x u64)
+//     [256, 256 + 3*MAX_CELLS*8)       fp64 merge buffer  part[3][norb][nE]
+//     [.., .. + 16 MiB)                block-partial histograms, as many copies of [nEp][3*norb] floats as fit
+// NOTE for maintainers: in HOST code the name g_static_scratch is only a handle for the runtime's symbol table, not
+// a device address.  Passing it (or &g_static_scratch[0]) to a kernel would hand the GPU a host-side address.  Host
+// code gets the real address from cudaGetSymbolAddress, once per device, in static_setup() below.
+namespace {
+
+constexpr size_t kStaticCountersOff = 0;
+constexpr size_t kStaticMergeOff = 256;
+constexpr size_t kStaticMergeBytes = (size_t)3 * TDOS_STATIC_MAX_CELLS * sizeof(double);
+constexpr size_t kStaticPartialOff = kStaticMergeOff + kStaticMergeBytes;
+constexpr size_t kStaticPartialBytes = (size_t)16 << 20;
+static_assert(kStaticPartialOff % 256 == 0, "partials start on a 256-byte boundary");
+static_assert(kStaticPartialOff + kStaticPartialBytes == (size_t)TDOS_STATIC_SCRATCH_BYTES, "header and layout agree");
+
+static __device__ __align__(256) unsigned char g_static_scratch[TDOS_STATIC_SCRATCH_BYTES];
+
+// what the first call on a device finds out and later calls reuse
+struct StaticDevice {
+    bool ready = false;
+    unsigned char* scratch = nullptr;   // device address of g_static_scratch on this device
+    int num_sms = 0;
+    size_t smem_optin = 0;
+    Variant var[4];                     // tdos_main for orbital blocks of 1, 2, 4, 8
+    int blocks_per_sm[4] = {0, 0, 0, 0};
+};
+constexpr int kStaticMaxDevices = 64;
+StaticDevice g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mutex;
+
+int mb_index(int MB) { return MB == 1 ? 0 : MB == 2 ? 1 : MB == 4 ? 2 : 3; }
+
+// Runs with `dev` current.  Nothing here allocates: symbol lookup, attribute queries, a function attribute.
+int static_setup(int dev, StaticDevice** out) {
+    if (dev < 0 || dev >= kStaticMaxDevices) return TDOS_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& sd = g_static_dev[dev];
+    if (!sd.ready) {
+        int major = 0, sms = 0, optin = 0;
+        CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major != 10) return TDOS_EARCH;
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CK(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        void* addr = nullptr;
+        CK(cudaGetSymbolAddress(&addr, g_static_scratch));
+        if (!addr) return TDOS_ECUDA;
+        const int mbs[4] = {1, 2, 4, 8};
+        for (int i = 0; i < 4; i++) {
+            sd.var[i] = variants(mbs[i])[0];   // 4 x 4 x 2 cubes per warp, groups of 2 lanes, 16 warps
+            CK(cudaFuncSetAttribute((const void*)sd.var[i].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&sd.blocks_per_sm[i], (const void*)sd.var[i].fn,
+                                                             sd.var[i].NWARP * 32, sd.var[i].smem));
+            if (sd.blocks_per_sm[i] < 1) return TDOS_ECUDA;
+        }
+        sd.scratch = static_cast<unsigned char*>(addr);
+        sd.num_sms = sms;
+        sd.smem_optin = (size_t)optin;
+        sd.ready = true;
+    }
+    *out = &sd;
+    return TDOS_OK;
+}
+
+}  // namespace
+
+extern "C" int tetra_dos_static(const int nk[3], int nb, int norb, const float* E, const float* W, int layout,
+                                const float* omega, int nE, float* dos, float* nos, void* cuda_stream) {
+    if (!nk || !E || !omega || !dos) return TDOS_EINVAL;
+    if (nk[0] < 1 || nk[1] < 1 || nk[2] < 1 || nb < 1 || norb < 1 || nE < 1 || nE > TDOS_MAX_NE) return TDOS_EINVAL;
+    if (layout != TDOS_AOS && layout != TDOS_SOA) return TDOS_EINVAL;
+    if (!W && norb != 1) return TDOS_EINVAL;
+    const long long nkt = (long long)nk[0] * nk[1] * nk[2];
+    if (nkt > 0x7fffffffLL) return TDOS_EINVAL;
+    const int nEp = rows_per_block(nE);
+    if ((long long)norb * nEp > TDOS_STATIC_MAX_CELLS) return TDOS_ESIZE;   // before anything touches the device
+
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    StaticDevice* sd = nullptr;
+    int rc = static_setup(dev, &sd);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    unsigned long long* counters = reinterpret_cast<unsigned long long*>(sd->scratch + kStaticCountersOff);
+    double* merged = reinterpret_cast<double*>(sd->scratch + kStaticMergeOff);
+    float* partial = reinterpret_cast<float*>(sd->scratch + kStaticPartialOff);
+
+    const int mi = mb_index(pick_mb(norb));
+    const Variant& v = sd->var[mi];
+    MainParams mp{};
+    mp.E = E;
+    mp.W = W;
+    mp.omega = omega;
+    if (layout == TDOS_AOS) {
+        mp.sEk = nb; mp.sEn = 1;
+        mp.sWk = (long long)nb * norb; mp.sWn = norb; mp.sWm = 1;
+    } else {
+        mp.sEk = 1; mp.sEn = nkt;
+        mp.sWk = 1; mp.sWn = (long long)norb * nkt; mp.sWm = nkt;
+    }
+    mp.N1 = nk[0]; mp.N2 = nk[1]; mp.N3 = nk[2];
+    mp.nb = nb; mp.norb = norb; mp.nE = nE;
+    mp.norb_in = norb;
+    mp.nEp = nEp;
+    mp.z_lo = 0; mp.z_hi = nk[2];
+    mp.unitW = (W == nullptr);
+    mp.ntx = (nk[0] + v.TX - 1) / v.TX;
+    mp.nty = (nk[1] + v.TY - 1) / v.TY;
+    mp.ntz = (nk[2] + v.TZ - 1) / v.TZ;
+    mp.nmb = (norb + v.MB - 1) / v.MB;
+    const long long items = (long long)mp.ntx * mp.nty * mp.ntz * nb * mp.nmb;
+    if (items > 0x7fffffffLL) return TDOS_EINVAL;
+    mp.n_items = (int)items;
+    mp.est = nullptr;   // this kernel runs unconditionally
+    mp.partial = partial;
+    mp.partial64 = nullptr;
+    mp.counters = counters;
+    mp.next_item = reinterpret_cast<unsigned int*>(counters + 3);
+
+    // one private histogram per block: as many blocks as histograms fit into the buffer, at most what the GPU holds
+    // and what the work needs (the size check above guarantees at least 42)
+    const size_t hist = (size_t)3 * norb * nEp;
+    long long grid = (long long)(kStaticPartialBytes / (hist * sizeof(float)));
+    const long long resident = (long long)sd->num_sms * sd->blocks_per_sm[mi];
+    const long long blocks_needed = (items + v.NWARP - 1) / v.NWARP;
+    if (grid > resident) grid = resident;
+    if (grid > blocks_needed) grid = blocks_needed;
+    if (grid < 1) grid = 1;
+
+    size_t smem = v.smem;
+    if (v.smem + (size_t)nE * sizeof(float) <= sd->smem_optin) {   // block-wide copy of omega in shared memory
+        mp.om_smem = 1;
+        smem += (size_t)nE * sizeof(float);
+    }
+
+    // the buffer still holds the previous call's sums: clear exactly what this call reads back
+    CK(cudaMemsetAsync(partial, 0, hist * (size_t)grid * sizeof(float), st));
+    CK(cudaMemsetAsync(counters, 0, 8 * sizeof(unsigned long long), st));
+    v.fn<<<(int)grid, v.NWARP * 32, smem, st>>>(mp);
+    CK(cudaGetLastError());
+    // the merge writes every element of part[3][norb][nE] that finalize reads: no clearing needed
+    const size_t cells = (size_t)3 * norb * nE;
+    tdos::tdos_merge<<<(int)((cells + 255) / 256), 256, 0, st>>>(partial, (int)grid, norb, nE, nEp, merged);
+    CK(cudaGetLastError());
+    const double V = 1.0 / (24.0 * (double)nk[0] * (double)nk[1] * (double)nk[2]);
+    tdos::tdos_finalize<<<norb, 1024, 0, st>>>(merged, norb, nE, V, dos, nos);
+    CK(cudaGetLastError());
+    return TDOS_OK;
+}
