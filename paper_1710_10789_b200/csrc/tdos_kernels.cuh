@@ -50,7 +50,7 @@ struct MainParams {
     // total: output row j < nsel is input orbital sel[j], row nsel (if total) is the sum over all norb_in input
     // orbitals, the rows up to norb are zero padding.  Otherwise output row = input orbital.
     int nsel, total, norb_in;
-    signed char sel[32];
+    short sel[32];
     int cplx;                    // W holds complex eigenvector elements a (re, im pairs), strides count pairs: b = |a|^2
     int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
     // kernel choice on the device (null: this kernel runs): {sum of window lengths in bins, (tetrahedron, band) pairs}

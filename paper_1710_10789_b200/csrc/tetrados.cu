@@ -139,6 +139,11 @@ struct tdos_plan {
     size_t smem_optin = 0;        // cudaDevAttrMaxSharedMemoryPerBlockOptin
     Variant var{};                // the main kernel (generation 5 when the orbitals allow it, else 3)
     Variant var_short{};          // adaptive plans: generation 3, better when the windows are a few bins only
+    // norb == 8 plans run tdos_main5<..., NORB = 8>, whose histogram layout is fixed at 8 rows; a selection of 9 rows
+    // (8 orbitals + total, padded to 12) needs the same tile with a run-time row count
+    Variant var_rows{};
+    bool has_var_rows = false;
+    int grid_rows = 0;
     bool adaptive = false;        // both kernels are enqueued; the device picks one per call (tdos_estimate)
     bool acc64 = false;           // tdos_plan_set_accumulation(TDOS_ACC_FP64): var64 runs, partials in fp64
     Variant var64{};
@@ -164,7 +169,7 @@ struct tdos_plan {
     int norb_alloc = 0;           // rows the scratch buffers hold: norb + 1 (selection + total), rounded up to 4
     int k_norb = 0, k_nout = 0;
     int sel_n = 0, sel_total = 0;
-    signed char sel[32] = {};
+    short sel[32] = {};
     float* dOm = nullptr;
     float* dDos = nullptr;
     float* dNos = nullptr;
@@ -292,6 +297,19 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
     }
     p->grid = p->num_sms * p->blocks_per_sm;
     p->nparts = p->grid;
+    if (gen == 5 && norb == 8) {
+        p->var_rows = variants5<0>()[sel];
+        int bps = 0;
+        e = setup(p->var_rows, &bps);
+        if (e != cudaSuccess || bps < 1) {
+            int rc = (e != cudaSuccess) ? cuda_fail(e, "kernel setup") : TDOS_ECUDA;
+            delete p;
+            return rc;
+        }
+        if (bps > p->blocks_per_sm) bps = p->blocks_per_sm;
+        p->has_var_rows = true;
+        p->grid_rows = p->num_sms * bps;
+    }
     // Without TDOS_KERNEL a plan on blocks of 8 orbitals carries both kernels: windows of a few bins only (config 5:
     // 3 bins on average) are served better by one record per tetrahedron (generation 3) than by three (generation 5).
     // Which one runs is decided per call on the device, from a sample of the windows (tdos_estimate).
@@ -351,7 +369,6 @@ static int check_common(const tdos_plan* p, const float* E, const float* W, int 
     return TDOS_OK;
 }
 
-// rows of one block's partial histogram: generation 5 flushes whole chunks of 4 bins
 // rows of one block's partial histogram: generation 5 flushes whole chunks of 4 bins; both kernels use this layout
 static int rows_per_block(int nE) { return (nE + 3) & ~3; }
 
@@ -424,8 +441,10 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     }
     long long items_main = 0;
     for (int which = 0; which < (pair ? 2 : 1); ++which) {
-        const Variant& v = p->acc64 ? p->var64 : which ? p->var_short : p->var;
-        const int vgrid = p->acc64 ? p->grid64 : which ? p->grid_short : p->grid;
+        // more than 8 output rows on a norb == 8 plan: the generation-5 kernel with a run-time row count
+        const bool rows = !which && p->has_var_rows && p->k_norb != 8;
+        const Variant& v = p->acc64 ? p->var64 : which ? p->var_short : rows ? p->var_rows : p->var;
+        const int vgrid = p->acc64 ? p->grid64 : which ? p->grid_short : rows ? p->grid_rows : p->grid;
         mp.ntx = (p->nk[0] + v.TX - 1) / v.TX;
         mp.nty = (p->nk[1] + v.TY - 1) / v.TY;
         mp.ntz = (z_hi - z_lo + v.TZ - 1) / v.TZ;
@@ -538,13 +557,13 @@ int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, c
                      const int* orbitals, int nsel, int want_total, float* dos, float* nos, int memspace, void* cuda_stream) {
     if (!p || !W || nsel < 0 || nsel > 32 || (nsel > 0 && !orbitals) || (nsel == 0 && !want_total)) return TDOS_EINVAL;
     for (int j = 0; j < nsel; j++)
-        if (orbitals[j] < 0 || orbitals[j] >= p->norb) return TDOS_EINVAL;
+        if (orbitals[j] < 0 || orbitals[j] >= p->norb || orbitals[j] > 32767) return TDOS_EINVAL;   // kept in 16 bits
     reset_call_state(p);
     const int nout = nsel + (want_total ? 1 : 0);
     if (nout > p->norb + 1) return TDOS_EINVAL;   // the scratch buffers hold norb + 1 rows
     p->sel_n = nsel;
     p->sel_total = want_total ? 1 : 0;
-    for (int j = 0; j < nsel; j++) p->sel[j] = (signed char)orbitals[j];
+    for (int j = 0; j < nsel; j++) p->sel[j] = (short)orbitals[j];
     p->k_nout = nout;
     // generation 5 works on whole blocks of 4 orbitals, at least 5 rows: the selection is padded with zero rows
     p->k_norb = (p->var.gen == 5 && !p->acc64) ? (nout <= 8 ? 8 : (nout + 3) & ~3) : nout;
@@ -637,7 +656,9 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
         // every slab is tiled from its own first plane, so a slab whose length is not a multiple of the tile's extent
         // in z ends in a layer of partly empty tiles: lengths are rounded to whole tiles (the short first slab, which
         // only has to start the kernels early, and the remainder at the end excepted)
-        const int tz = p->var.TZ;
+        // (the largest tile extent among the kernels that may run this call; all are powers of two)
+        int tz = p->acc64 ? p->var64.TZ : p->var.TZ;
+        if (!p->acc64 && p->adaptive && p->var_short.TZ > tz) tz = p->var_short.TZ;
         for (int i = 0; i < ns && zb[nslab] < N3; i++) {
             acc += sizes[i] * scale;
             int z = (int)(acc / plane_bytes + 0.5);

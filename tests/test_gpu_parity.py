@@ -523,6 +523,58 @@ def test_orbital_selection_small_cases():
             plan.tetra_dos_select(dE, dW, dOm, [], False, ddos, dnos)         # nothing asked for
 
 
+@pytest.mark.parametrize("host", [False, True])
+def test_all_eight_orbitals_plus_total_on_an_eight_orbital_plan(cache_dir, host):
+    """Nine rows (every orbital of the 8-orbital model and the total) on a norb == 8 plan: one row more than the
+    compile-time 8-row kernel holds, so the plan switches to the same tile with a run-time row count (12 padded rows);
+    still generation 5 (round-2 advisor finding: the rows came back scrambled)."""
+    import torch
+    cfg = wl.CONFIGS["paper60"]
+    E, W, om, ref = _full_ref("paper60", cache_dir)
+    sel = [3, 0, 1, 2, 7, 6, 5, 4]
+    want = {"dos": np.concatenate([ref["dos"][sel], ref["dos"].sum(axis=0, keepdims=True)]),
+            "nos": np.concatenate([ref["nos"][sel], ref["nos"].sum(axis=0, keepdims=True)])}
+    with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
+        if host:
+            dos, nos = np.full((9, cfg.nE), np.nan, np.float32), np.full((9, cfg.nE), np.nan, np.float32)
+            plan.tetra_dos_select(E, W, om, sel, True, dos, nos, memspace=binding.TDOS_HOST)
+        else:
+            dev = torch.device("cuda:0")
+            dE, dW, dOm = (torch.from_numpy(a).to(dev) for a in (E, W, om))
+            ddos = torch.full((9, cfg.nE), float("nan"), device=dev)
+            dnos = torch.full((9, cfg.nE), float("nan"), device=dev)
+            plan.tetra_dos_select(dE, dW, dOm, sel, True, ddos, dnos)
+            torch.cuda.synchronize()
+            dos, nos = ddos.cpu().numpy(), dnos.cpu().numpy()
+        assert plan.last_counters()["kernel"] == 5
+        assert_parity(want, dos, nos, "8 orbitals + total")
+        dos8, nos8 = run_gpu(E, W, cfg.nk, om, plan=plan)          # the 8-row kernel again
+        assert_parity(ref, dos8, nos8, "full call after 9 rows")
+
+
+def test_orbital_index_above_127():
+    """The selection is kept in 16 bits: orbital 130 of a 132-orbital problem (round-2 advisor finding: an 8-bit
+    field wrapped negative and read out of bounds)."""
+    import torch
+    dev = torch.device("cuda:0")
+    nk, nb, norb, nE = (3, 3, 2), 1, 132, 40
+    E, W = wl.random_bands(nk, nb, norb, seed=132)
+    om = wl.omega_grid(-1.2, 1.3, nE)
+    ref = oracle.tetra_dos(E, W, nk, om)
+    sel = [130, 5, 127, 128]
+    want = {"dos": np.concatenate([ref["dos"][sel], ref["dos"].sum(axis=0, keepdims=True)]),
+            "nos": np.concatenate([ref["nos"][sel], ref["nos"].sum(axis=0, keepdims=True)])}
+    dE, dW, dOm = (torch.from_numpy(a).to(dev) for a in (E, W, om))
+    ddos = torch.full((5, nE), float("nan"), device=dev)
+    dnos = torch.full((5, nE), float("nan"), device=dev)
+    with binding.Plan(nk, nb, norb, nE) as plan:
+        plan.tetra_dos_select(dE, dW, dOm, sel, True, ddos, dnos)
+        torch.cuda.synchronize()
+        assert_parity(want, ddos.cpu().numpy(), dnos.cpu().numpy(), "orbital 130")
+        with pytest.raises(binding.TdosError):
+            plan.tetra_dos_select(dE, dW, dOm, [132], False, ddos, dnos)
+
+
 def test_fp64_accumulation_reaches_the_output_rounding_floor(cache_dir):
     """with tdos_plan_set_accumulation(TDOS_ACC_FP64) the single-precision corner
     weights are summed in fp64 everywhere.  On the band-structure configs the result then agrees with the fp64 oracle to
