@@ -38,6 +38,7 @@
  * first enqueues tdos_estimate, which samples the windows (E1, E4) of 2048 cubes on the device, then both main
  * kernels; the one that suits the windows runs (tdos_main below 7 energies per window on average, tdos_main5
  * above), the other returns at once.  Nothing is decided on the host and nothing is remembered between calls.
+ * (In TDOS_HOST mode the sample is taken from the first staged z-slab, the only planes on the device at that time.)
  * Environment variables read at plan creation, for experiments only: TDOS_KERNEL=3|5 forces one kernel, TDOS_TILE=<index>
  * picks another compiled tile shape, TDOS_BLOCKS_PER_SM=<n> lowers the number of resident blocks.
  *
@@ -143,7 +144,7 @@ int tetra_dos_complex(tdos_plan* p, const float* E, const float* A, int layout, 
 /*
  * Orbital selection plus total ("the five Fe 3d orbitals ... and the total density of states" of an
  * 8-orbital model; reading G15: total = sum over ALL orbitals).  Rows of dos / nos:
- *     j < nsel : orbital orbitals[j] (0-based, each < norb, any order, repeats allowed),
+ *     j < nsel : orbital orbitals[j] (0-based, each < norb and <= 32767, any order, repeats allowed),
  *     j = nsel : sum over all norb orbitals, present if want_total != 0.
  * dos, nos are [nsel + (want_total != 0)][nE]; nsel <= 32, at most norb + 1 rows; nsel = 0 with want_total gives the
  * total alone.  W must not be NULL; `orbitals` is a HOST array in both memory spaces.  Everything else as tetra_dos.
@@ -157,13 +158,14 @@ int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, c
  * The step before the path, on the device (Eq. 1, :37-39: the tight-binding Hamiltonian H(k) is "diagonalised
  * to obtain band energies E_n(k) and eigenvector elements a_n^m(k)"; :289: the best case is input that already
  * resides in GPU memory): batched Hermitian eigensolver for plans with nb == norb <= 8 (the paper's model: 8).
- *   H  in  device, nk*nb*nb complex numbers as (re, im) float pairs, H[ik][i][j] row-major, Hermitian
+ *   H  in  device, nk*nb*nb complex numbers as (re, im) float pairs, H[ik][i][j] row-major, Hermitian: only the upper
+ *      triangle (j >= i) and the real part of the diagonal are read, the rest is taken as its conjugate
  *   E  out device [nk][nb], ascending per k-point                                     (TDOS_AOS layout of tetra_dos)
  *   A  out device [nk][nb][nb][2]: A[ik][n][m] = a_n^m(k), component m of eigenvector n (TDOS_AOS layout of
  *      tetra_dos_complex), normalised, phase arbitrary
  * so that  tetra_eigh(p, H, E, A, s); tetra_dos_complex(p, E, A, TDOS_AOS, ...)  goes from H(k) to the DOS without a
- * host round trip.  Cyclic Jacobi, fp64 arithmetic like the host LAPACK call it replaces, results rounded to the fp32
- * arrays the path consumes.  Asynchronous on `cuda_stream`.  TDOS_EINVAL if nb != norb or nb > 8.
+ * host round trip.  Cyclic Jacobi, fp64 arithmetic like the host LAPACK call it replaces (sweeps until the off-diagonal
+ * norm is below 1e-12 of the matrix norm, at most 10), results rounded to the fp32 arrays the path consumes.  Asynchronous on `cuda_stream`.  TDOS_EINVAL if nb != norb or nb > 8.
  */
 int tetra_eigh(tdos_plan* p, const float* H, float* E, float* A, void* cuda_stream);
 

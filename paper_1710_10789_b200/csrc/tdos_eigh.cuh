@@ -10,8 +10,9 @@
 // The pairs of a round are compile-time constants (fully unrolled), so all register indices are static; the column
 // part of H <- J^H (H J) and V <- V J is local to a lane, the row part is one exchange of rows between the two lanes
 // of a pair (shuffles).  The arithmetic is fp64 (as the host LAPACK call it replaces; the results are rounded to the
-// fp32 arrays the path consumes), a fixed number of sweeps (the method converges quadratically; 10 sweeps are ample
-// for order 8).  Eigenvalues are written in ascending order with their eigenvectors.
+// fp32 arrays the path consumes).  Sweeps stop when every matrix of the warp has an off-diagonal Frobenius norm below
+// 1e-12 of its own norm, at most `sweeps` (10) of them (the method converges quadratically; 4-6 are typical for
+// order 8).  Only the upper triangle of H is read.  Eigenvalues are written in ascending order with their eigenvectors.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -115,13 +116,35 @@ __global__ void __launch_bounds__(128) tdos_eigh8(const EighParams P) {
         vr[j] = (j == r) ? 1.0 : 0.0;
         vi[j] = 0.0;
     }
+    // Only the upper triangle of the input is read: H_rj for j >= r, its conjugate for j < r, a real diagonal.  An input
+    // that is Hermitian only to fp32 rounding (assembled on the device) is thereby made exactly Hermitian, which the
+    // rotations below rely on (they read H_pq from row p and never look at H_qp).
     if (live && r < nb) {
-        const float2* row = P.H + (mat * nb + r) * nb;
+        const float2* M = P.H + mat * nb * nb;
 #pragma unroll
         for (int j = 0; j < 8; j++)
-            if (j < nb) { const float2 z = __ldg(row + j); hr[j] = z.x; hi[j] = z.y; }
+            if (j < nb) {
+                const float2 z = __ldg(j >= r ? M + r * nb + j : M + j * nb + r);
+                hr[j] = z.x;
+                hi[j] = j > r ? z.y : j < r ? -z.y : 0.0;
+            }
     }
     for (int sweep = 0; sweep < P.sweeps; ++sweep) {
+        // Convergence: stop once, for every matrix of the warp, the off-diagonal part is below 1e-12 of the matrix in
+        // the Frobenius norm (the outputs are rounded to fp32, 6e-8).  Padded rows (r >= nb) count as zero.
+        double off = 0.0, all = 0.0;
+#pragma unroll
+        for (int j = 0; j < 8; j++) {
+            const double a2 = (r < nb) ? hr[j] * hr[j] + hi[j] * hi[j] : 0.0;
+            all += a2;
+            if (j != r) off += a2;
+        }
+#pragma unroll
+        for (int d = 1; d < 8; d <<= 1) {
+            off += __shfl_xor_sync(mask, off, d);
+            all += __shfl_xor_sync(mask, all, d);
+        }
+        if (!__any_sync(mask, live && off > 1e-24 * all)) break;
         jacobi_round<0>(hr, hi, vr, vi, r, base, mask);
         jacobi_round<1>(hr, hi, vr, vi, r, base, mask);
         jacobi_round<2>(hr, hi, vr, vi, r, base, mask);

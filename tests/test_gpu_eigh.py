@@ -74,6 +74,27 @@ def test_random_hermitian_matrices_every_order(nb):
             plan.tetra_eigh(torch.from_numpy(H).cuda(), dE, dA)
 
 
+def test_only_the_upper_triangle_is_read():
+    """include/tetrados.h: the lower triangle and the imaginary part of the diagonal are ignored, so an input that is
+    Hermitian only up to rounding (or not at all below the diagonal) gives the eigenpairs of the Hermitian matrix its
+    upper triangle defines -- identical to those of the clean input."""
+    rng = np.random.default_rng(8)
+    nk, nb = (4, 3, 3), 8
+    n = int(np.prod(nk))
+    M = rng.normal(size=(n, nb, nb)) + 1j * rng.normal(size=(n, nb, nb))
+    H = ((M + M.conj().transpose(0, 2, 1)) / 2).astype(np.complex64)
+    dirty = H.copy()
+    il = np.tril_indices(nb, -1)
+    dirty[:, il[0], il[1]] = (rng.normal(size=(n, len(il[0]))) + 1j * rng.normal(size=(n, len(il[0])))).astype(np.complex64)
+    dirty[:, np.arange(nb), np.arange(nb)] += 1j * rng.normal(size=(n, nb)).astype(np.float32)
+    with binding.Plan(nk, nb, nb, 16) as plan:
+        dE, dA = _gpu_eigh(plan, H)
+        dE2, dA2 = _gpu_eigh(plan, dirty)
+    assert torch.equal(dE, dE2) and torch.equal(torch.view_as_real(dA), torch.view_as_real(dA2))
+    Eo, _ = oracle.eigh_bands(H)
+    assert np.abs(dE.cpu().numpy() - Eo).max() <= 2e-6
+
+
 def test_hamiltonian_to_dos_without_leaving_the_device():
     """H(k) -> tetra_eigh -> tetra_dos_complex against oracle.eigh_bands -> oracle.tetra_dos (fp32 inputs as in every
     other config).  The eigensolver works in fp64 and rounds to fp32 like the oracle's side does; the two sets of fp32
