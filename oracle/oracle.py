@@ -155,7 +155,8 @@ def eigh_bands(H):
     """PAPER.md Eq. 1 (:37-39): H(k) "is diagonalised to obtain band energies E_n(k) and eigenvector elements a_n^m(k)".
     H[ik][nb][nb] complex Hermitian -> (E[ik][nb] ascending, W[ik][n][m] = |a_n^m(k)|^2), both float64.  The
     diagonalisation itself is the library routine numpy.linalg.eigh (LAPACK zheevd) in complex128; nothing else is
-    done here.  Pinned in tests/test_oracle_pins.py by H a = E a, orthonormality and a closed-form 2 x 2 case."""
+    done here.  Pinned in tests/test_oracle_pins.py by a closed-form 2 x 2 case, the two sum rules of |a|^2 and, for the
+    [n][m] orientation of W, by the Hellmann-Feynman derivative dE_n/dH_mm = |a_n^m|^2 of its own eigenvalues."""
     H = np.asarray(H).astype(np.complex128)
     w, U = np.linalg.eigh(H)                      # U[ik][m][n]: column n is eigenvector n
     W = (U.real ** 2 + U.imag ** 2).transpose(0, 2, 1)

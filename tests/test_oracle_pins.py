@@ -490,3 +490,28 @@ def test_eigh_bands_pins(oracle_lib):
     assert np.abs(np.einsum("kij,kjn->kin", H.astype(np.complex128), U) - U * w[:, None, :]).max() < 1e-13
     Eb, Wb = wl.tb8_bands(nk, threads=1)
     assert np.abs(E - Eb).max() < 2e-6 and np.abs(W - Wb).max() < 2e-5      # complex64 H against complex128 H
+
+
+@pytest.mark.parametrize("nb,seed", [(3, 1), (8, 2)])
+def test_eigh_bands_orientation_by_hellmann_feynman(oracle_lib, nb, seed):
+    """Which index of W is the band and which the orbital (Eq. 1 -> E_n(k), a_n^m(k), :37-39; Eq. 3
+    b_mn = a* a, :47) is pinned without reference to any eigenvector routine: by the Hellmann-Feynman theorem
+    dE_n / dH_mm = |a_n^m|^2, so a central difference of the n-th EIGENVALUE returned by eigh_bands under a shift of
+    the m-th diagonal element of H must reproduce W[n][m].  |U|^2 of a 2 x 2 unitary is symmetric, so only orders >= 3
+    can tell W[n][m] from W[m][n]; a transposed W fails this by O(1)."""
+    rng = np.random.default_rng(seed)
+    M = rng.normal(size=(nb, nb)) + 1j * rng.normal(size=(nb, nb))
+    H = (M + M.conj().T) / 2
+    E0, W = oracle_lib.eigh_bands(H[None])
+    assert np.diff(E0[0]).min() > 1e-2                         # well separated levels: the derivative exists
+    h = 1e-5
+    D = np.empty((nb, nb))                                     # D[n][m] = dE_n / dH_mm
+    for m in range(nb):
+        Hp, Hm = H.copy(), H.copy()
+        Hp[m, m] += h
+        Hm[m, m] -= h
+        Ep, _ = oracle_lib.eigh_bands(Hp[None])
+        Em, _ = oracle_lib.eigh_bands(Hm[None])
+        D[:, m] = (Ep[0] - Em[0]) / (2 * h)
+    assert np.abs(D - W[0]).max() < 1e-7
+    assert np.abs(D - W[0].T).max() > 1e-2                     # the pin can see the orientation
