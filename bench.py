@@ -67,6 +67,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg4", choices=sorted(wl.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--layout", default="aos", choices=["aos", "soa"],
+                    help="aos: E[ik][n], W[ik][n][m] (default); soa: E[n][ik], W[n][m][ik] (k fastest; 1 GPU only)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -138,7 +140,7 @@ def oracle_sample_planes(cfg) -> int:
 
 
 def run_oracle_sample(cfg, E, W, om, reps: int = 1, warmup: int = 0, single_core: bool = False):
-    """Time the fp64 oracle, as it stands, on the sample.  Returns (seconds per rep, n_tb, n_eval, cores, text).
+    """Time the fp64 oracle, as it stands, on the sample.  Returns (median seconds per rep, n_tb, n_eval, cores, text).
     single_core: one thread on 1/8 of the sample's planes (comparable in spirit with the paper's single-core
     CPU reference)."""
     import oracle
@@ -158,7 +160,17 @@ def run_oracle_sample(cfg, E, W, om, reps: int = 1, warmup: int = 0, single_core
     text = ("oracle.tetra_dos(windowed=True: Eq. 12-14 inside (E1,E4), Eq. 15 by step+prefix), fp64, OpenMP over cubes, "
             "on the cubes of z-planes [0,%d) of %s (%d of %d cubes), all %d energies"
             % (planes, cfg.name, hi, int(np.prod(cfg.nk)), cfg.nE))
-    return float(np.mean(times)), res["n_tb"], res["n_eval"], cores, text
+    return float(np.median(times)), res["n_tb"], res["n_eval"], cores, text
+
+
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def reference_arm(args, cfg, rank: int):
@@ -172,20 +184,22 @@ def reference_arm(args, cfg, rank: int):
         "impl": "reference", "metric": "tetra*band*omega evaluations/sec", "value": value, "unit": "eval/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3,
         "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(cfg, args.gpus),
+        "config": workload_config(cfg, args.gpus, args.layout),
         "effective_evals_per_s": n_eval / sec,
-        "cpu_baseline": {"value": value, "unit": "eval/s", "cores": cores, "kind": "oracle", "sample": text},
+        "cpu_baseline": {"value": value, "unit": "eval/s", "cores": cores, "kind": "oracle", "sample": text,
+                         "timing": "median of %d after %d warm-up" % (args.steps, args.warmup), "cpu": cpu_model()},
         "e2e": {"value": value, "unit": "eval/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
 
 
-def workload_config(cfg, n_gpus: int) -> dict:
+def workload_config(cfg, n_gpus: int, layout: str = "aos") -> dict:
     return {"workload": "%s: %s, Nk=%dx%dx%d, nb=%d, norb=%d, nE=%d on [%g,%g]" % (
                 cfg.name, "seeded 8-orbital tetragonal tight-binding" if cfg.model == "tb8" else "simple-cubic cosine band",
                 cfg.nk[0], cfg.nk[1], cfg.nk[2], cfg.nb, cfg.norb, cfg.nE, cfg.omega_min, cfg.omega_max),
-            "nk": list(cfg.nk), "nb": cfg.nb, "norb": cfg.norb, "nE": cfg.nE, "layout": "AoS E[ik][n], W[ik][n][m]",
+            "nk": list(cfg.nk), "nb": cfg.nb, "norb": cfg.norb, "nE": cfg.nE,
+            "layout": "AoS E[ik][n], W[ik][n][m]" if layout == "aos" else "SoA E[n][ik], W[n][m][ik]",
             "parallelism": "1 GPU" if n_gpus == 1 else "z-slabs over %d GPUs + all-reduce of fp64 partials" % n_gpus}
 
 
@@ -233,6 +247,14 @@ def main():
     unitW = cfg.model == "cosine"
     dE = torch.from_numpy(E).to(dev)
     dW = None if unitW else torch.from_numpy(W).to(dev)
+    layout = binding.TDOS_AOS
+    if args.layout == "soa":   # the same numbers with k fastest (north_star (1)); converted on the device
+        if world > 1:
+            raise SystemExit("--layout soa is a 1-GPU measurement (the z-slab staging of the N > 1 leg slices AoS arrays)")
+        layout = binding.TDOS_SOA
+        dE = dE.t().contiguous()
+        if dW is not None:
+            dW = dW.permute(1, 2, 0).contiguous()
     dOm = torch.from_numpy(om).to(dev)
     dos = torch.zeros((norb, nE), device=dev)
     nos = torch.zeros((norb, nE), device=dev)
@@ -242,7 +264,7 @@ def main():
 
     def step():
         if world == 1:
-            plan.tetra_dos(dE, dW, dOm, dos, nos)
+            plan.tetra_dos(dE, dW, dOm, dos, nos, layout=layout)
         else:   # partial over this rank's z-slab -> ONE all-reduce (the path's only exchange step) -> finalize
             multigpu.sharded_step(plan, dE, dW, dOm, N3, rank, world, part, dos, nos, dist.all_reduce)
 
@@ -285,8 +307,8 @@ def main():
     # ---- e2e: the same step through the C-ABI with HOST (pinned) buffers
     e2e = None
     if not args.no_e2e:
-        hE = torch.from_numpy(E).pin_memory()
-        hW = None if unitW else torch.from_numpy(W).pin_memory()
+        hE = (torch.from_numpy(E) if layout == binding.TDOS_AOS else dE.cpu()).pin_memory()
+        hW = None if unitW else (torch.from_numpy(W) if layout == binding.TDOS_AOS else dW.cpu()).pin_memory()
         hOm = torch.from_numpy(om).pin_memory()
         hdos = torch.zeros((norb, nE)).pin_memory()
         hnos = torch.zeros((norb, nE)).pin_memory()
@@ -294,7 +316,7 @@ def main():
 
         def e2e_step():
             if world == 1:
-                plan.tetra_dos(hE, hW, hOm, hdos, hnos, memspace=binding.TDOS_HOST)
+                plan.tetra_dos(hE, hW, hOm, hdos, hnos, layout=layout, memspace=binding.TDOS_HOST)
                 return
             # each rank stages its own z-slab plus the halo plane, then partial -> all-reduce -> finalize
             a, b = z_lo * plane, z_hi * plane
@@ -378,11 +400,14 @@ def main():
     fl = fl_paper
     achieved = fl / (main_ms * 1e-3) / 1e12
     bytes_alg = 4.0 * N1 * N2 * N3 * nb * (1 + (0 if unitW else norb)) + 8.0 * norb * nE
-    traffic = NCU_TRAFFIC_BYTES.get((cfg.name, gen))
+    traffic = NCU_TRAFFIC_BYTES.get((cfg.name, gen)) if layout == binding.TDOS_AOS else None
     roofline = {"bound": "alu", "kernel": "tdos_main5" if gen == 5 else "tdos_main", "achieved": achieved, "peak": peak,
                 "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic[0] if traffic else None,
                 "traffic_source": (traffic[1] + " (constant from that ncu capture, not measured in this run)") if traffic else None,
                 "flop_model": "SURVEY.md 8(d): F_eval = 40 + 18 norb, F_tb = 40 + 5 norb, units counted by the kernel",
+                "note": "achieved/frac count the ALGORITHMIC flops of the paper's formulation (the figure the 0.60 target is "
+                        "stated in), not instructions executed: the kernel's own formulation needs fewer flops, and the "
+                        "fraction of the FP32 peak it actually keeps busy is frac_kernel_formulation",
                 "frac_kernel_formulation": fl_kernel / (main_ms * 1e-3) / 1e12 / peak,
                 "flops_kernel_formulation_per_launch": fl_kernel,
                 "frac_paper_formulation": fl_paper / (main_ms * 1e-3) / 1e12 / peak,
@@ -400,7 +425,7 @@ def main():
         "metric": "tetra*band*omega evaluations/sec", "value": n_tb * nE / (ms_per_step * 1e-3), "unit": "eval/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
         "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": dict(workload_config(cfg, world), l2="inputs (%.0f MB) larger than L2 (126 MB), no flush" % (bytes_alg / 1e6)
+        "config": dict(workload_config(cfg, world, args.layout), l2="inputs (%.0f MB) larger than L2 (126 MB), no flush" % (bytes_alg / 1e6)
                        if bytes_alg > 126e6 else "inputs fit in L2; L2 not flushed between steps",
                        tile=list(info["tile"]), grid=info["grid"], threads=info["threads"], smem=info["smem"]),
         "effective_evals_per_s": n_eval / (ms_per_step * 1e-3), "dos_grids_per_s": 1e3 / ms_per_step,
@@ -410,10 +435,14 @@ def main():
     }
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        sec, s_tb, s_eval, cores, text = run_oracle_sample(cfg, E, W, om)
+        # 3 warm-ups (OpenMP team start-up; first touch of the thread-private histograms, which stops only once the
+        # C library serves them from its heap instead of fresh mappings: the first ~4 calls run 1.5x slower) + median
+        # of 5, like the --impl reference arm's default warm-up (mean of five runs for the CPU reference)
+        sec, s_tb, s_eval, cores, text = run_oracle_sample(cfg, E, W, om, reps=5, warmup=3)
         line["cpu_baseline"] = {"value": s_tb * nE / sec, "unit": "eval/s", "cores": cores, "kind": "oracle",
-                                "sample": text, "seconds": sec, "effective_evals_per_s": s_eval / sec}
-        sec1, t_tb, t_eval, _, text1 = run_oracle_sample(cfg, E, W, om, single_core=True)
+                                "sample": text, "seconds": sec, "effective_evals_per_s": s_eval / sec,
+                                "timing": "median of 5 after 3 warm-ups", "cpu": cpu_model()}
+        sec1, t_tb, t_eval, _, text1 = run_oracle_sample(cfg, E, W, om, reps=5, warmup=3, single_core=True)
         line["cpu_baseline"]["single_core"] = {"value": t_tb * nE / sec1, "unit": "eval/s", "cores": 1, "sample": text1,
                                                "seconds": sec1, "effective_evals_per_s": t_eval / sec1}
     if rank == 0:

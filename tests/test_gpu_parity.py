@@ -247,6 +247,22 @@ def test_cfg4_full_size_headline(cache_dir):
     _full_config("cfg4", cache_dir, expect_kernel=5)
 
 
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_soa_layout(name, cache_dir):
+    """north_star (1) names a k-major SoA layout (E[n][ik], W[n][m][ik]): the same full-size comparison with the
+    inputs transposed, device mode, generation 5; work counters equal to the oracle's."""
+    cfg = wl.CONFIGS[name]
+    E, W, om, ref = _full_ref(name, cache_dir)
+    Es, Ws = wl.to_soa(E, W)
+    with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
+        dos, nos = run_gpu(Es, Ws, cfg.nk, om, layout=binding.TDOS_SOA, plan=plan)
+        cnt = plan.last_counters()
+    del Es, Ws
+    d, en = assert_parity(ref, dos, nos, name + " SoA")
+    assert cnt["kernel"] == 5 and cnt["n_tb"] == ref["n_tb"] and cnt["n_eval"] == ref["n_eval"]
+    print("%s SoA dDOS %.2e dN %.2e" % (name, d, en))
+
+
 def test_cfg5_full_size_host_inputs(cache_dir):
     """windows of 3 bins: the device picks tdos_main (generation 3) on every call"""
     _full_config("cfg5", cache_dir, host=True, calls=2, expect_kernel=3)
