@@ -39,8 +39,10 @@
  * kernels; the one that suits the windows runs (tdos_main below 7 energies per window on average, tdos_main5
  * above), the other returns at once.  Nothing is decided on the host and nothing is remembered between calls.
  * (In TDOS_HOST mode the sample is taken from the first staged z-slab, the only planes on the device at that time.)
- * Environment variables read at plan creation, for experiments only: TDOS_KERNEL=3|5 forces one kernel, TDOS_TILE=<index>
- * picks another compiled tile shape, TDOS_BLOCKS_PER_SM=<n> lowers the number of resident blocks.
+ * Environment variables read at plan creation, for tests and experiments only: TDOS_KERNEL=3|5 forces one kernel,
+ * TDOS_TILE=<index> forces one of the compiled tile shapes (generation 5: 0 = 4x4x2, 1 = 2x2x8 cubes per warp;
+ * generation 3 on blocks of 8 orbitals: 0 = 2-lane groups, 1 and 2 = the short-window kernels).  A library built with
+ * -DTDOS_EXPERIMENTS carries more shapes and reads TDOS_BLOCKS_PER_SM (DESIGN.md section 4 and the experiments logs).
  *
  * Ownership: the caller owns every array; the library never frees them and does not retain them
  * past the call (device mode: past completion of the work queued on `stream`).  A plan owns all

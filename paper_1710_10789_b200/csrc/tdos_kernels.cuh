@@ -408,13 +408,18 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
                 sW[k * WST + m] = (m0 + m < norb) ? load_out_weight(p, ik * p.sWk + (long long)n * p.sWn, m0 + m) : 0.0f;
             }
-        } else {                   // k contiguous (SoA): k fastest across lanes
-            for (int q = lane; q < PK * MB; q += 32) {
-                const int k = q % PK, m = q / PK;
+        } else {                   // k contiguous (SoA): lane = k-point, its MB orbitals fetched together (index arithmetic
+                                   // once per k-point, MB independent loads in flight; neighbouring lanes read neighbouring k)
+            for (int k = lane; k < PK; k += 32) {
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 const int gx = (x0 + px) % p.N1, gy = (y0 + py) % p.N2, gz = (z0 + pz) % p.N3;
                 const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
-                sW[k * WST + m] = (m0 + m < norb) ? load_out_weight(p, ik * p.sWk + (long long)n * p.sWn, m0 + m) : 0.0f;
+                const long long wbase = ik * p.sWk + (long long)n * p.sWn;
+                float v[MB];
+#pragma unroll
+                for (int m = 0; m < MB; m++) v[m] = (m0 + m < norb) ? load_out_weight(p, wbase, m0 + m) : 0.0f;
+#pragma unroll
+                for (int m = 0; m < MB; m++) sW[k * WST + m] = v[m];
             }
         }
         __syncwarp();

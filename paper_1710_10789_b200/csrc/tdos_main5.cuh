@@ -520,10 +520,24 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main5(const MainParams p) 
                     v = __ldg(reinterpret_cast<const float4*>(p.W + ik * p.sWk + (long long)n * p.sWn + m0 + 4 * part4));
                 *reinterpret_cast<float4*>(sW + k * WST + 4 * part4) = v;
             }
-        } else {                   // any strides: AoS with norb % 4 != 0, or SoA (k fastest across lanes)
-            const bool kfast = p.sWm != 1;
+        } else if (p.sWm != 1) {   // SoA (k contiguous): lane = k-point, its 8 orbitals fetched together -- the index
+                                   // arithmetic is done once per k-point and 8 independent loads are in flight per lane;
+                                   // neighbouring lanes read neighbouring k (runs of PX floats per orbital plane)
+            for (int k = lane; k < PK; k += 32) {
+                const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
+                int gx = x0 + px, gy = y0 + py, gz = z0 + pz;
+                while (gx >= p.N1) gx -= p.N1; while (gy >= p.N2) gy -= p.N2; while (gz >= p.N3) gz -= p.N3;
+                const long long ik = gx + (long long)p.N1 * (gy + (long long)p.N2 * gz);
+                const long long wbase = ik * p.sWk + (long long)n * p.sWn;
+                float v[MB];
+#pragma unroll
+                for (int m = 0; m < MB; m++) v[m] = (m0 + m < norb) ? load_out_weight(p, wbase, m0 + m) : 0.0f;
+                *reinterpret_cast<float4*>(sW + k * WST) = make_float4(v[0], v[1], v[2], v[3]);
+                *reinterpret_cast<float4*>(sW + k * WST + 4) = make_float4(v[4], v[5], v[6], v[7]);
+            }
+        } else {                   // AoS that does not qualify for whole float4s (selection, complex input, alignment)
             for (int qi = lane; qi < PK * MB; qi += 32) {
-                const int k = kfast ? qi % PK : qi / MB, m = kfast ? qi / PK : qi % MB;
+                const int k = qi / MB, m = qi % MB;
                 const int px = k % PX, py = (k / PX) % PY, pz = k / (PX * PY);
                 int gx = x0 + px, gy = y0 + py, gz = z0 + pz;
                 while (gx >= p.N1) gx -= p.N1; while (gy >= p.N2) gy -= p.N2; while (gz >= p.N3) gz -= p.N3;

@@ -76,12 +76,16 @@ Variant make_variant5() {
     return v;
 }
 
-// v5 configurations compiled in (TDOS_TILE=<index> selects another one for experiments); norb == 8 has its own
-// instantiation with compile-time histogram offsets
+// v5 configurations compiled in: the two tiles a default plan can pick (TDOS_TILE=<index> forces one); norb == 8 has
+// its own instantiation with compile-time histogram offsets.  A build with -DTDOS_EXPERIMENTS adds the other shapes
+// that were measured in DESIGN.md's experiments logs.
 template <int NORB>
 std::vector<Variant> variants5() {
-    return {make_variant5<4, 4, 2, 16, NORB>(), make_variant5<2, 2, 8, 16, NORB>(), make_variant5<4, 2, 4, 16, NORB>(),
-            make_variant5<4, 4, 2, 12, NORB>(), make_variant5<4, 4, 1, 16, NORB>()};
+    return {make_variant5<4, 4, 2, 16, NORB>(), make_variant5<2, 2, 8, 16, NORB>()
+#ifdef TDOS_EXPERIMENTS
+            , make_variant5<4, 2, 4, 16, NORB>(), make_variant5<4, 4, 2, 12, NORB>(), make_variant5<4, 4, 1, 16, NORB>()
+#endif
+    };
 }
 
 template <int MB, int TX, int TY, int TZ, int GL, int NWARP>
@@ -109,16 +113,26 @@ Variant variant64(int MB) {
 // orbital-block width: the smallest of 1, 2, 4, 8 that holds norb (8 for norb > 8, several blocks)
 int pick_mb(int norb) { return norb <= 1 ? 1 : norb <= 2 ? 2 : norb <= 4 ? 4 : 8; }
 
-// Configurations compiled in: tile of cubes per warp, lanes per group, warps per block.
-// TDOS_TILE=<index> selects another one for experiments.
+// Configurations compiled in: tile of cubes per warp, lanes per group, warps per block.  [0] is the kernel of plans
+// that do not qualify for generation 5; blocks of 8 orbitals also have the two short-window kernels.
+// TDOS_TILE=<index> forces one of them; -DTDOS_EXPERIMENTS adds the other shapes of the experiments logs.
 template <int MB>
 std::vector<Variant> variants_for() {
-    return {make_variant<MB, 4, 4, 2, 2, 16>(), make_variant<MB, 4, 4, 2, 4, 16>(), make_variant<MB, 4, 4, 4, 2, 12>(),
-            make_variant<MB, 4, 4, 4, 4, 12>(), make_variant<MB, 4, 4, 2, 2, 20>(),
-            // groups of ONE lane (chunks of 2 bins): the short-window kernel of plans that carry two
-            make_variant<MB, 4, 4, 2, 1, 16>(), make_variant<MB, 2, 2, 8, 1, 16>()};
+    std::vector<Variant> v = {make_variant<MB, 4, 4, 2, 2, 16>()};
+    if constexpr (MB == 8) {
+        // groups of ONE lane (chunks of 2 bins): the short-window kernel of plans that carry two
+        v.push_back(make_variant<MB, 4, 4, 2, 1, 16>());
+        v.push_back(make_variant<MB, 2, 2, 8, 1, 16>());
+    }
+#ifdef TDOS_EXPERIMENTS
+    v.push_back(make_variant<MB, 4, 4, 2, 4, 16>());
+    v.push_back(make_variant<MB, 4, 4, 4, 2, 12>());
+    v.push_back(make_variant<MB, 4, 4, 4, 4, 12>());
+    v.push_back(make_variant<MB, 4, 4, 2, 2, 20>());
+#endif
+    return v;
 }
-constexpr int kShortVariant = 5, kShortVariantZ8 = 6;   // indices into variants_for<8>()
+constexpr int kShortVariant = 1, kShortVariantZ8 = 2;   // indices into variants_for<8>()
 
 std::vector<Variant> variants(int MB) {
     switch (MB) {
@@ -291,10 +305,12 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
         delete p;
         return rc;
     }
-    if (const char* s = getenv("TDOS_BLOCKS_PER_SM")) {   // experiments only (include/tetrados.h)
+#ifdef TDOS_EXPERIMENTS
+    if (const char* s = getenv("TDOS_BLOCKS_PER_SM")) {   // fewer resident blocks, for occupancy experiments
         int b = atoi(s);
         if (b >= 1 && b < p->blocks_per_sm) p->blocks_per_sm = b;
     }
+#endif
     p->grid = p->num_sms * p->blocks_per_sm;
     p->nparts = p->grid;
     if (gen == 5 && norb == 8) {
