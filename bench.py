@@ -69,6 +69,11 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layout", default="aos", choices=["aos", "soa"],
                     help="aos: E[ik][n], W[ik][n][m] (default); soa: E[n][ik], W[n][m][ik] (k fastest; 1 GPU only)")
+    ap.add_argument("--op", default="dos", choices=["dos", "eigh", "h2dos", "weights", "select", "table2"],
+                    help="dos: the hot path (the contract's JSON line).  The others time the SURVEY 8(f) operations on "
+                         "one GPU and print their own JSON line(s): eigh (tetra_eigh), h2dos (H(k) -> eigh -> DOS on the "
+                         "device), weights (tetra_weights), select (5 orbitals + total), table2 (the paper's Table II "
+                         "shapes: device-resident, host buffers, one-shot)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -194,6 +199,146 @@ def reference_arm(args, cfg, rank: int):
     print(json.dumps(line), flush=True)
 
 
+def hbm_peak_gbs():
+    """(GB/s, source): the measured copy bandwidth of this pool's B200s, else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def run_ops(args, cfg):
+    """--op eigh | h2dos | weights | select | table2: the SURVEY.md 8(f) operations on one GPU, timed with CUDA events
+    after 3 warm-ups, inputs resident on the device unless the line says otherwise; one JSON line per operation."""
+    import torch
+    from paper_1710_10789_b200 import binding
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    peak, peak_src = hbm_peak_gbs()
+    K, Wm = args.steps, max(args.warmup, 3)
+
+    def timed(fn, steps=K):
+        for _ in range(Wm):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(steps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / steps
+
+    def out(line):
+        line.update({"n_gpus": 1, "steps": K, "warmup": Wm, "data": "synthetic"})
+        print(json.dumps(line), flush=True)
+
+    nk, nb, norb, nE = cfg.nk, cfg.nb, cfg.norb, cfg.nE
+    nkt = int(np.prod(nk))
+    if args.op in ("eigh", "h2dos"):
+        assert cfg.model == "tb8", "--op eigh / h2dos need an 8-orbital config"
+        H = wl.tb8_hamiltonian(nk)
+        dH = torch.from_numpy(H).to(dev)
+        dE = torch.empty((nkt, nb), device=dev)
+        dA = torch.empty((nkt, nb, nb), dtype=torch.complex64, device=dev)
+        dOm = torch.from_numpy(wl.omega_grid(cfg.omega_min, cfg.omega_max, nE)).to(dev)
+        dos, nos = torch.empty((norb, nE), device=dev), torch.empty((norb, nE), device=dev)
+        with binding.Plan(nk, nb, norb, nE) as plan:
+            ms_eigh = timed(lambda: plan.tetra_eigh(dH, dE, dA))
+            bytes_alg = nkt * (nb * nb * 8 + nb * 4 + nb * nb * 8)
+            roof = {"bound": "hbm", "kernel": "tdos_eigh8", "achieved": bytes_alg / ms_eigh / 1e6, "peak": peak, "unit": "GB/s",
+                    "frac": bytes_alg / ms_eigh / 1e6 / peak, "traffic": None, "peak_source": peak_src,
+                    "bytes_alg": bytes_alg,
+                    "note": "algorithmic bytes = H in + E, A out; the kernel is fp64-ALU work (cyclic Jacobi, 8 lanes per "
+                            "matrix), so the HBM fraction is a lower-bound reference, not a target"}
+            if args.op == "eigh":
+                out({"op": "eigh", "metric": "8x8 Hermitian eigenproblems/sec", "value": nkt / (ms_eigh * 1e-3), "unit": "matrices/s",
+                     "ms_per_step": ms_eigh, "higher_is_better": True, "dtype": "f64", "config": workload_config(cfg, 1),
+                     "roofline": roof, "gpu_launches": K})
+                return
+            ms_dos = timed(lambda: plan.tetra_dos_complex(dE, torch.view_as_real(dA), dOm, dos, nos))
+
+            def chain():
+                plan.tetra_eigh(dH, dE, dA)
+                plan.tetra_dos_complex(dE, torch.view_as_real(dA), dOm, dos, nos)
+            ms_chain = timed(chain)
+            out({"op": "h2dos", "metric": "H(k) -> DOS grids/sec (device resident)", "value": 1e3 / ms_chain, "unit": "grids/s",
+                 "ms_per_step": ms_chain, "higher_is_better": True, "dtype": "f64 eigensolver, f32 DOS",
+                 "config": workload_config(cfg, 1), "eigh_ms": ms_eigh, "tetra_dos_complex_ms": ms_dos,
+                 "h_bytes": int(H.nbytes), "gpu_launches": K * 6,
+                 "note": "PAPER.md:289 best case: the Hamiltonian is on the device and nothing returns to the host but DOS, N"})
+        return
+    E, W, om = wl.make_inputs(cfg, args.cache)
+    dE, dOm = torch.from_numpy(E).to(dev), torch.from_numpy(om).to(dev)
+    dW = None if cfg.model == "cosine" else torch.from_numpy(W).to(dev)
+    if args.op == "weights":
+        nW = 16
+        en = torch.from_numpy(wl.omega_grid(cfg.omega_min, cfg.omega_max, nW)).to(dev)
+        wk = torch.empty((nW, nb, nkt), device=dev)
+        dwk = torch.empty((nW, nb, nkt), device=dev)
+        with binding.Plan(nk, nb, norb, nE) as plan:
+            ms = timed(lambda: plan.tetra_weights(dE, en, wk, dwk))
+        bytes_alg = E.nbytes + 2 * wk.numel() * 4           # E read once, wk and dwk written once
+        out({"op": "weights", "metric": "per-k integration weights/sec", "value": 2 * wk.numel() / (ms * 1e-3), "unit": "weights/s",
+             "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "config": dict(workload_config(cfg, 1), nW=nW),
+             "roofline": {"bound": "hbm", "kernel": "tdos_kweights", "achieved": bytes_alg / ms / 1e6, "peak": peak, "unit": "GB/s",
+                          "frac": bytes_alg / ms / 1e6 / peak, "traffic": None, "peak_source": peak_src, "bytes_alg": bytes_alg,
+                          "note": "24 scalar red.global.add per output element plus the two memsets; untuned"},
+             "gpu_launches": K})
+        return
+    if args.op == "select":
+        sel = [0, 2, 3, 5, 7][:max(1, min(5, norb - 1))]
+        dos, nos = torch.empty((len(sel) + 1, nE), device=dev), torch.empty((len(sel) + 1, nE), device=dev)
+        dosf, nosf = torch.empty((norb, nE), device=dev), torch.empty((norb, nE), device=dev)
+        with binding.Plan(nk, nb, norb, nE) as plan:
+            ms_sel = timed(lambda: plan.tetra_dos_select(dE, dW, dOm, sel, True, dos, nos))
+            ms_full = timed(lambda: plan.tetra_dos(dE, dW, dOm, dosf, nosf))
+        out({"op": "select", "metric": "DOS grids/sec, %d orbitals + total" % len(sel), "value": 1e3 / ms_sel, "unit": "grids/s",
+             "ms_per_step": ms_sel, "higher_is_better": True, "dtype": "f32", "config": workload_config(cfg, 1),
+             "all_orbitals_ms": ms_full, "gpu_launches": K * 5})
+        return
+    # ---- table2: PAPER.md Table II (:315-320) shapes, 8 bands, 1024 energies, 5 orbitals + total (PAPER.md:279)
+    rows = []
+    for shape in ((10, 10, 10), (20, 20, 10), (25, 25, 25), (60, 60, 10)):
+        n = int(np.prod(shape))
+        E, W = wl.tb8_bands(shape)
+        om = wl.omega_grid(-6.0, 4.0, 1024)
+        dE, dW, dOm = (torch.from_numpy(a).to(dev) for a in (E, W, om))
+        hE, hW, hOm = (torch.from_numpy(a).pin_memory() for a in (E, W, om))
+        sel = [0, 2, 3, 5, 7]
+        dos, nos = torch.empty((6, 1024), device=dev), torch.empty((6, 1024), device=dev)
+        hdos, hnos = torch.empty((6, 1024)).pin_memory(), torch.empty((6, 1024)).pin_memory()
+        odos, onos = np.empty((8, 1024), np.float32), np.empty((8, 1024), np.float32)
+        with binding.Plan(shape, 8, 8, 1024) as plan:
+            ms_dev = timed(lambda: plan.tetra_dos_select(dE, dW, dOm, sel, True, dos, nos), steps=max(K, 20))
+            t = []
+            for r in range(Wm + 5):
+                t0 = time.perf_counter()
+                plan.tetra_dos_select(hE, hW, hOm, sel, True, hdos, hnos, memspace=binding.TDOS_HOST)
+                t.append((time.perf_counter() - t0) * 1e3)
+            ms_host = float(np.median(t[Wm:]))
+        ms_shot = None
+        if shape[0] == shape[1] == shape[2]:   # tetra_dos_simple takes cubic grids only
+            t = []
+            for r in range(Wm + 5):   # one-shot: plan creation + H2D + kernels + D2H + destroy, pageable host arrays
+                t0 = time.perf_counter()
+                binding.tetra_dos_simple(E, W, shape[0], 8, 8, -6.0, 4.0, 1024, odos, onos)
+                t.append((time.perf_counter() - t0) * 1e3)
+            ms_shot = float(np.median(t[Wm:]))
+        rows.append({"n_k": n, "grid": list(shape), "evaluations_paper": n * 6 * 8 * 1024,
+                     "device_resident_ms": ms_dev, "host_buffers_ms": ms_host, "one_shot_simple_ms": ms_shot,
+                     "paper_gtx970_ms": {1000: [24.4, 98.7], 4000: [81.8, 169.4], 15625: [318.9, 451.4], 36000: [732.0, 936.7]}[n]})
+    out({"op": "table2", "metric": "run time per DOS grid, Table II shapes", "unit": "ms", "higher_is_better": False,
+         "dtype": "f32", "rows": rows,
+         "note": "5 orbitals + total, 8 bands, 1024 energies on the seeded 8-orbital model (the paper's FeSe parameters are not "
+                 "available). device_resident = the paper's best case (:289), host_buffers = tetra_dos_select with pinned host "
+                 "arrays on an existing plan, one_shot_simple = tetra_dos_simple (cubic grids only; all 8 orbitals; plan "
+                 "creation, H2D from pageable memory, kernels, D2H, destroy: the paper's worst case, :287). "
+                 "paper_gtx970_ms = [best, worst] of Table II, another machine: context only"})
+
+
 def workload_config(cfg, n_gpus: int, layout: str = "aos") -> dict:
     return {"workload": "%s: %s, Nk=%dx%dx%d, nb=%d, norb=%d, nE=%d on [%g,%g]" % (
                 cfg.name, "seeded 8-orbital tetragonal tight-binding" if cfg.model == "tb8" else "simple-cubic cosine band",
@@ -219,6 +364,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         reference_arm(args, cfg, rank)
+        return 0
+    if args.op != "dos":
+        if rank == 0:
+            run_ops(args, cfg)
         return 0
 
     import torch
