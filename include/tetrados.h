@@ -159,7 +159,8 @@ int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, c
 /*
  * The step before the path, on the device (Eq. 1, :37-39: the tight-binding Hamiltonian H(k) is "diagonalised
  * to obtain band energies E_n(k) and eigenvector elements a_n^m(k)"; :289: the best case is input that already
- * resides in GPU memory): batched Hermitian eigensolver for plans with nb == norb <= 8 (the paper's model: 8).
+ * resides in GPU memory): batched Hermitian eigensolver for plans with nb == norb <= 16 (the paper's model: 8; "16
+ * orbitals correspond to the largest models ... currently considered", :269).
  *   H  in  device, nk*nb*nb complex numbers as (re, im) float pairs, H[ik][i][j] row-major, Hermitian: only the upper
  *      triangle (j >= i) and the real part of the diagonal are read, the rest is taken as its conjugate
  *   E  out device [nk][nb], ascending per k-point                                     (TDOS_AOS layout of tetra_dos)
@@ -167,7 +168,8 @@ int tetra_dos_select(tdos_plan* p, const float* E, const float* W, int layout, c
  *      tetra_dos_complex), normalised, phase arbitrary
  * so that  tetra_eigh(p, H, E, A, s); tetra_dos_complex(p, E, A, TDOS_AOS, ...)  goes from H(k) to the DOS without a
  * host round trip.  Cyclic Jacobi, fp64 arithmetic like the host LAPACK call it replaces (sweeps until the off-diagonal
- * norm is below 1e-12 of the matrix norm, at most 10), results rounded to the fp32 arrays the path consumes.  Asynchronous on `cuda_stream`.  TDOS_EINVAL if nb != norb or nb > 8.
+ * norm is below 1e-12 of the matrix norm, at most 10; 14 for orders above 8), results rounded to the fp32 arrays the
+ * path consumes; 8 lanes per matrix up to order 8, 16 lanes above.  Asynchronous on `cuda_stream`.  TDOS_EINVAL if nb != norb or nb > 16.
  */
 int tetra_eigh(tdos_plan* p, const float* H, float* E, float* A, void* cuda_stream);
 

@@ -24,7 +24,7 @@ struct EighParams {
     float* E;            // [nmat][nb] ascending
     float2* A;           // [nmat][nb][nb]: A[i][n][m] = component m of eigenvector n
     long long nmat;
-    int nb;              // 1..8
+    int nb;              // 1..8 (tdos_eigh8), 9..16 (tdos_eigh_n<16>)
     int sweeps;
 };
 
@@ -166,6 +166,142 @@ __global__ void __launch_bounds__(128) tdos_eigh8(const EighParams P) {
         if (rank < nb && r < nb) {
             if (r == 0) P.E[mat * nb + rank] = (float)lam[c];
             P.A[(mat * nb + rank) * nb + r] = make_float2((float)vr[c], (float)vi[c]);   // component m = r of eigenvector `rank`
+        }
+    }
+}
+
+// ---- orders 9..16 ("16 orbitals correspond to the largest models of iron-based superconductors currently
+// considered"): the same method with N = 16 lanes per matrix (2 matrices per warp), N - 1 rounds of N/2 disjoint
+// rotations per sweep.  The rotations of a round are taken one after the other (parameters from 4 broadcasts, column
+// update of H and V at once), so only one set of rotation parameters is live beside the 4 N doubles of state; a lane
+// keeps the parameters of the pair its own row belongs to for the row half.  Disjoint pairs do not touch each other's
+// H_pp, H_qq, H_pq, so taking them in sequence gives the same rotations as taking them together.
+template <int N>
+__host__ __device__ constexpr int rrn_player(int s, int pos) {   // circle method: position 0 fixed, 1..N-1 rotate
+    return pos == 0 ? 0 : 1 + (pos - 1 + s) % (N - 1);
+}
+
+template <int N, int S>
+__device__ __forceinline__ void jacobi_round_n(double (&hr)[N], double (&hi)[N], double (&vr)[N], double (&vi)[N], int r, int base) {
+    constexpr unsigned mask = 0xffffffffu;
+    double cc = 1.0, ss = 0.0, fr = 1.0, fi = 0.0;
+    int partner = r;
+    bool is_p = true;
+#pragma unroll
+    for (int k = 0; k < N / 2; k++) {
+        const int p = rrn_player<N>(S, k), q = rrn_player<N>(S, N - 1 - k);
+        const double a = __shfl_sync(mask, hr[p], base + p);     // H_pp
+        const double b = __shfl_sync(mask, hr[q], base + q);     // H_qq
+        const double gr = __shfl_sync(mask, hr[q], base + p);    // H_pq = |H_pq| e^{i phi}
+        const double gi = __shfl_sync(mask, hi[q], base + p);
+        const double g2 = gr * gr + gi * gi;
+        double c = 1.0, s = 0.0, er = 1.0, ei = 0.0;
+        if (g2 > 1e-280) {
+            const double ig = 1.0 / sqrt(g2);
+            const double tau = (b - a) * (0.5 * ig);
+            const double t = copysign(1.0, tau) / (fabs(tau) + sqrt(1.0 + tau * tau));
+            c = 1.0 / sqrt(1.0 + t * t);
+            s = t * c;
+            er = gr * ig;
+            ei = gi * ig;
+        }
+        // columns: X[:, p'] = c X[:, p] - s e^{-i phi} X[:, q],  X[:, q'] = s X[:, p] + c e^{-i phi} X[:, q]   (X = H, V)
+        {
+            const double xr = hr[p], xi = hi[p];
+            const double yr = hr[q] * er + hi[q] * ei, yi = hi[q] * er - hr[q] * ei;
+            hr[p] = c * xr - s * yr; hi[p] = c * xi - s * yi;
+            hr[q] = s * xr + c * yr; hi[q] = s * xi + c * yi;
+        }
+        {
+            const double xr = vr[p], xi = vi[p];
+            const double yr = vr[q] * er + vi[q] * ei, yi = vi[q] * er - vr[q] * ei;
+            vr[p] = c * xr - s * yr; vi[p] = c * xi - s * yi;
+            vr[q] = s * xr + c * yr; vi[q] = s * xi + c * yi;
+        }
+        if (r == p || r == q) {
+            cc = c; ss = s; fr = er; fi = ei;
+            partner = (r == p) ? q : p;
+            is_p = (r == p);
+        }
+    }
+    // rows of H: X[p', :] = c X[p, :] - s e^{+i phi} X[q, :],  X[q', :] = s X[p, :] + c e^{+i phi} X[q, :]
+#pragma unroll
+    for (int j = 0; j < N; j++) {
+        const double tr = __shfl_sync(mask, hr[j], base + partner), ti = __shfl_sync(mask, hi[j], base + partner);
+        const double pr = is_p ? hr[j] : tr, pi = is_p ? hi[j] : ti;
+        const double qr0 = is_p ? tr : hr[j], qi0 = is_p ? ti : hi[j];
+        const double qr = qr0 * fr - qi0 * fi, qi = qr0 * fi + qi0 * fr;
+        hr[j] = is_p ? cc * pr - ss * qr : ss * pr + cc * qr;
+        hi[j] = is_p ? cc * pi - ss * qi : ss * pi + cc * qi;
+    }
+}
+
+template <int N, int S>
+struct JacobiSweep {
+    static __device__ __forceinline__ void run(double (&hr)[N], double (&hi)[N], double (&vr)[N], double (&vi)[N], int r, int base) {
+        jacobi_round_n<N, S>(hr, hi, vr, vi, r, base);
+        JacobiSweep<N, S + 1>::run(hr, hi, vr, vi, r, base);
+    }
+};
+template <int N>
+struct JacobiSweep<N, N - 1> {
+    static __device__ __forceinline__ void run(double (&)[N], double (&)[N], double (&)[N], double (&)[N], int, int) {}
+};
+
+template <int N>
+__global__ void __launch_bounds__(128) tdos_eigh_n(const EighParams P) {
+    static_assert(N == 16, "lanes per matrix");
+    const int lane = threadIdx.x & 31, r = lane & (N - 1), base = lane & ~(N - 1);
+    const long long mat = (blockIdx.x * (long long)blockDim.x + threadIdx.x) / N;
+    const bool live = mat < P.nmat;
+    const unsigned mask = 0xffffffffu;
+    const int nb = P.nb;
+    double hr[N], hi[N], vr[N], vi[N];
+#pragma unroll
+    for (int j = 0; j < N; j++) {
+        hr[j] = (j == r && r >= nb) ? 1e30 * (1 + r) : 0.0;   // padding: decoupled levels far above, sorted last
+        hi[j] = 0.0;
+        vr[j] = (j == r) ? 1.0 : 0.0;
+        vi[j] = 0.0;
+    }
+    if (live && r < nb) {   // upper triangle only, mirrored (see tdos_eigh8)
+        const float2* M = P.H + mat * nb * nb;
+#pragma unroll
+        for (int j = 0; j < N; j++)
+            if (j < nb) {
+                const float2 z = __ldg(j >= r ? M + r * nb + j : M + j * nb + r);
+                hr[j] = z.x;
+                hi[j] = j > r ? z.y : j < r ? -z.y : 0.0;
+            }
+    }
+    for (int sweep = 0; sweep < P.sweeps; ++sweep) {
+        double off = 0.0, all = 0.0;
+#pragma unroll
+        for (int j = 0; j < N; j++) {
+            const double a2 = (r < nb) ? hr[j] * hr[j] + hi[j] * hi[j] : 0.0;
+            all += a2;
+            if (j != r) off += a2;
+        }
+#pragma unroll
+        for (int d = 1; d < N; d <<= 1) {
+            off += __shfl_xor_sync(mask, off, d);
+            all += __shfl_xor_sync(mask, all, d);
+        }
+        if (!__any_sync(mask, live && off > 1e-24 * all)) break;
+        JacobiSweep<N, 0>::run(hr, hi, vr, vi, r, base);
+    }
+    double lam[N];
+#pragma unroll
+    for (int c = 0; c < N; c++) lam[c] = __shfl_sync(mask, hr[c], base + c);
+    if (!live) return;
+#pragma unroll
+    for (int c = 0; c < N; c++) {
+        int rank = 0;
+#pragma unroll
+        for (int d = 0; d < N; d++) rank += (lam[d] < lam[c] || (lam[d] == lam[c] && d < c)) ? 1 : 0;
+        if (rank < nb && r < nb) {
+            if (r == 0) P.E[mat * nb + rank] = (float)lam[c];
+            P.A[(mat * nb + rank) * nb + r] = make_float2((float)vr[c], (float)vi[c]);
         }
     }
 }

@@ -763,7 +763,7 @@ int tetra_weights(tdos_plan* p, const float* E, int layout, const float* energie
 
 int tetra_eigh(tdos_plan* p, const float* H, float* E, float* A, void* cuda_stream) {
     if (!p || !H || !E || !A) return TDOS_EINVAL;
-    if (p->nb != p->norb || p->nb > 8) return TDOS_EINVAL;   // square problems of order <= 8 (the paper's model: 8)
+    if (p->nb != p->norb || p->nb > 16) return TDOS_EINVAL;   // square problems of order <= 16
     ON_DEVICE(p->device);
     tdos::EighParams ep{};
     ep.H = reinterpret_cast<const float2*>(H);
@@ -771,9 +771,15 @@ int tetra_eigh(tdos_plan* p, const float* H, float* E, float* A, void* cuda_stre
     ep.A = reinterpret_cast<float2*>(A);
     ep.nmat = (long long)p->nk[0] * p->nk[1] * p->nk[2];
     ep.nb = p->nb;
-    ep.sweeps = 10;
-    const long long threads = ep.nmat * 8;
-    tdos::tdos_eigh8<<<(unsigned)((threads + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(ep);
+    if (p->nb <= 8) {        // 8 lanes per matrix
+        ep.sweeps = 10;
+        const long long threads = ep.nmat * 8;
+        tdos::tdos_eigh8<<<(unsigned)((threads + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(ep);
+    } else {                 // orders 9..16: 16 lanes per matrix
+        ep.sweeps = 14;
+        const long long threads = ep.nmat * 16;
+        tdos::tdos_eigh_n<16><<<(unsigned)((threads + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(ep);
+    }
     CK(cudaGetLastError());
     return TDOS_OK;
 }

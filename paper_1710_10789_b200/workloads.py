@@ -170,6 +170,25 @@ def tb8_hamiltonian(nk, chunk: int = 65536) -> np.ndarray:
     return out
 
 
+def random_tb_hamiltonian(nk, norb: int, seed: int, hop: float = 0.35) -> np.ndarray:
+    """A seeded generic tight-binding Hamiltonian of any order (input generator for the eigensolver tests at orders
+    above 8): H(k) = T0 + sum_d (T_d e^{2 pi i k_d} + h.c.), T0 Hermitian with a spread diagonal, T_d
+    random complex nearest-neighbour hoppings.  Smooth and periodic in k; H[ik][norb][norb] complex64, exactly
+    Hermitian after the cast."""
+    rng = np.random.default_rng(seed)
+    T0 = rng.normal(size=(norb, norb)) + 1j * rng.normal(size=(norb, norb))
+    T0 = 0.25 * (T0 + T0.conj().T) + np.diag(np.linspace(-2.0, 2.0, norb))
+    Td = hop * (rng.normal(size=(3, norb, norb)) + 1j * rng.normal(size=(3, norb, norb)))
+    k = kgrid(nk)                                            # [nk][3] in units of the reciprocal lattice vectors
+    ph = np.exp(2j * np.pi * k)                              # [nk][3]
+    H = np.broadcast_to(T0, (k.shape[0], norb, norb)).copy()
+    for d in range(3):
+        hopd = ph[:, d, None, None] * Td[d][None]
+        H += hopd + hopd.conj().transpose(0, 2, 1)
+    H = 0.5 * (H + H.conj().transpose(0, 2, 1))
+    return H.astype(np.complex64)
+
+
 def tb8_bands(nk, threads: int | None = None, chunk: int = 16384):
     """Configs 2-5: E[ik][8] ascending (fp32), W[ik][n][m] = |U[m][n]|^2 (fp32).
     H(k) = s*(H_raw(k) - c) - 1 with c, s from the Nk=16 spectrum so that the

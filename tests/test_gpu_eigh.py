@@ -48,9 +48,10 @@ def test_eigenvalues_and_orbital_weights_of_the_seeded_model():
     assert np.abs(R).max() <= 3e-6
 
 
-@pytest.mark.parametrize("nb", [1, 2, 3, 5, 8])
+@pytest.mark.parametrize("nb", [1, 2, 3, 5, 8, 9, 12, 16])
 def test_random_hermitian_matrices_every_order(nb):
-    """orders below 8 are padded inside the kernel; degenerate and diagonal matrices included"""
+    """orders below 8 (below 16 for the 16-lane kernel of orders 9..16, PAPER.md:269) are padded inside the kernel;
+    degenerate and diagonal matrices included"""
     rng = np.random.default_rng(100 + nb)
     nk = (5, 4, 3)
     n = int(np.prod(nk))
@@ -69,6 +70,10 @@ def test_random_hermitian_matrices_every_order(nb):
     assert np.abs(R).max() <= 5e-6
     G = np.einsum("knm,kpm->knp", A, A.conj())
     assert np.abs(G - np.eye(nb)).max() <= 2e-6
+    if nb == 16:
+        with binding.Plan(nk, 17, 17, 16) as plan:        # above the largest order
+            with pytest.raises(binding.TdosError):
+                plan.tetra_eigh(torch.zeros((n, 17, 17), dtype=torch.complex64).cuda(), dE, dA)
     with binding.Plan(nk, nb, nb + 1, 16) as plan:        # not a square problem
         with pytest.raises(binding.TdosError):
             plan.tetra_eigh(torch.from_numpy(H).cuda(), dE, dA)
@@ -123,3 +128,38 @@ def test_hamiltonian_to_dos_without_leaving_the_device():
     assert (np.abs(n - ref["nos"])[big] / ref["nos"][big]).max() <= 1e-5
     assert (np.abs(n - ref["nos"]) / nmax)[~big].max() <= 1e-8
     print("H -> DOS on the device: dDOS %.2e, dN/N (N > 1e-3) %.2e" % (d, (np.abs(n - ref["nos"])[big] / ref["nos"][big]).max()))
+
+
+def test_sixteen_orbital_hamiltonian_to_dos_on_the_device():
+    """PAPER.md:269: "16 orbitals correspond to the largest models of iron-based superconductors currently considered".
+    A seeded 16-orbital tight-binding H(k) -> tetra_eigh (16 lanes per matrix) -> tetra_dos_complex (two orbital
+    blocks) against oracle.eigh_bands -> oracle.tetra_dos, with the tolerances of the 8-orbital chain test."""
+    nk, norb, nE = (10, 8, 6), 16, 600
+    H = wl.random_tb_hamiltonian(nk, norb, seed=16)
+    assert np.array_equal(H, H.conj().transpose(0, 2, 1))
+    Eo, Wo = oracle.eigh_bands(H)
+    om = wl.omega_grid(float(Eo.min()) - 0.3, float(Eo.max()) + 0.3, nE)
+    ref = oracle.tetra_dos(Eo.astype(np.float32), Wo.astype(np.float32), nk, om, nthreads=oracle.max_threads())
+    dev = torch.device("cuda:0")
+    dOm = torch.from_numpy(om).to(dev)
+    dos = torch.full((norb, nE), float("nan"), device=dev)
+    nos = torch.full((norb, nE), float("nan"), device=dev)
+    with binding.Plan(nk, norb, norb, nE) as plan:
+        dE, dA = _gpu_eigh(plan, H)
+        plan.tetra_dos_complex(dE, torch.view_as_real(dA), dOm, dos, nos)
+        torch.cuda.synchronize()
+    E = dE.cpu().numpy().astype(np.float64)
+    A = dA.cpu().numpy().astype(np.complex128)
+    assert np.abs(E - Eo).max() <= 2e-6
+    G = np.einsum("knm,kpm->knp", A, A.conj())
+    assert np.abs(G - np.eye(norb)).max() <= 2e-6
+    R = np.einsum("kij,knj->kni", H.astype(np.complex128), A) - A * E[:, :, None]
+    assert np.abs(R).max() <= 5e-6
+    d, _, _ = errors(ref, dos.cpu().numpy(), None)
+    assert d <= TOL_DOS
+    n = nos.cpu().numpy().astype(np.float64)
+    nmax = ref["nos"][:, -1:]
+    big = ref["nos"] > 1e-3 * nmax
+    assert (np.abs(n - ref["nos"])[big] / ref["nos"][big]).max() <= 1e-5
+    assert (np.abs(n - ref["nos"]) / nmax)[~big].max() <= 1e-8
+
