@@ -535,6 +535,17 @@ def main():
         fp64_acc = {"ms_per_step": f0.elapsed_time(f1) / 3, "main_kernel_ms": plan.kernel_ms(3)[0],
                     "what": "tdos_plan_set_accumulation(TDOS_ACC_FP64): single-precision corner weights, every sum after "
                             "them in fp64 (generation 3 kernel, fp64 block partials)"}
+        plan.set_accumulation(True, weights_fp64=True)
+        for _ in range(2):
+            step()
+        torch.cuda.synchronize()
+        f0.record()
+        for _ in range(2):
+            step()
+        f1.record()
+        torch.cuda.synchronize()
+        fp64_acc["all_fp64_ms_per_step"] = f0.elapsed_time(f1) / 2
+        fp64_acc["all_fp64_what"] = "TDOS_ACC_FP64_ALL: corner weights in double precision too (agrees with the fp64 oracle to 1e-14)"
         plan.set_accumulation(False)
 
     # ---- roofline of the dominant kernel (tdos_main): FP32 ALU

@@ -106,9 +106,13 @@ int tdos_plan_create(tdos_plan** out, int device, const int nk[3], int nb, int n
  * block partials, the Eq.-15 step histogram, merge, prefix sum) is fp64; slower (about 3x on config 4), results agree
  * with the fp64 oracle to ~1e-7 relative instead of ~1e-6.  Allocates a second, fp64 set of block
  * partials the first time the mode is chosen (TDOS_ENOMEM if that fails); waits for the plan's last call.
+ * TDOS_ACC_FP64_ALL: the corner weights of Eq. 11-14 are evaluated in double precision as well (true divisions instead
+ * of rcp.approx), so the whole path after the fp32 inputs is fp64; the fp64 shares of tetra_dos_partial then agree
+ * with the fp64 oracle to ~1e-12 relative (the fp32 outputs of tetra_dos still round to 6e-8).  Slowest mode.
  */
 #define TDOS_ACC_FP32 0
 #define TDOS_ACC_FP64 1
+#define TDOS_ACC_FP64_ALL 2
 int tdos_plan_set_accumulation(tdos_plan* p, int mode);
 
 /* Free a plan and everything it owns.  NULL is a no-op.  Synchronises the plan's streams first. */

@@ -12,7 +12,7 @@ from . import build as _build
 
 TDOS_OK, TDOS_EINVAL, TDOS_ENOMEM, TDOS_ECUDA, TDOS_EARCH, TDOS_ESIZE = 0, -1, -2, -3, -4, -5
 TDOS_AOS, TDOS_SOA = 0, 1
-TDOS_ACC_FP32, TDOS_ACC_FP64 = 0, 1
+TDOS_ACC_FP32, TDOS_ACC_FP64, TDOS_ACC_FP64_ALL = 0, 1, 2
 TDOS_DEVICE, TDOS_HOST = 0, 1
 TDOS_MAX_NE = 65534
 TDOS_STATIC_MAX_CELLS = 32768   # tetra_dos_static: norb * (nE rounded up to 4) it accepts
@@ -98,9 +98,11 @@ class Plan:
         _check(lib.tdos_plan_create(C.byref(self._h), self.device, arr, self.nb, self.norb, self.nE_max),
                "tdos_plan_create")
 
-    def set_accumulation(self, fp64: bool):
-        """tdos_plan_set_accumulation(): fp64 sums after the single-precision corner weights."""
-        _check(load().tdos_plan_set_accumulation(self._h, TDOS_ACC_FP64 if fp64 else TDOS_ACC_FP32), "tdos_plan_set_accumulation")
+    def set_accumulation(self, fp64, weights_fp64: bool = False):
+        """tdos_plan_set_accumulation(): fp64 sums after the single-precision corner weights (PAPER.md:271);
+        weights_fp64 (or fp64 == TDOS_ACC_FP64_ALL): the corner weights in double precision too."""
+        mode = TDOS_ACC_FP64_ALL if (weights_fp64 or fp64 == TDOS_ACC_FP64_ALL) else (TDOS_ACC_FP64 if fp64 else TDOS_ACC_FP32)
+        _check(load().tdos_plan_set_accumulation(self._h, mode), "tdos_plan_set_accumulation")
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

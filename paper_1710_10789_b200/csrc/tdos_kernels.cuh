@@ -53,6 +53,7 @@ struct MainParams {
     short sel[32];
     int cplx;                    // W holds complex eigenvector elements a (re, im pairs), strides count pairs: b = |a|^2
     int om_smem;                 // tdos_main5: the launch has room for a copy of omega behind the warps' slices
+    int w64;                     // tdos_main<..., ACC64 = true> only: corner weights in double precision too
     // kernel choice on the device (null: this kernel runs): {sum of window lengths in bins, (tetrahedron, band) pairs}
     // of a sample, written by tdos_estimate earlier on the stream; see wanted_generation()
     const unsigned long long* est;
@@ -296,6 +297,23 @@ struct Acc64 {
                 D[1][m] = fma(bm, db, D[1][m]);
                 T[0][m] = fma(bm, wa, T[0][m]);
                 T[1][m] = fma(bm, wb, T[1][m]);
+            }
+        }
+    }
+    // the same with double-precision weights, [l][energy]
+    __device__ __forceinline__ void project64(const float* __restrict__ sW, const unsigned (&cc)[4], const double (&w)[4][2],
+                                              const double (&dw)[4][2]) {
+#pragma unroll
+        for (int l = 0; l < 4; l++) {
+            float b[MB];
+            load_b<MB>(sW + cc[l], b);
+#pragma unroll
+            for (int m = 0; m < MB; m++) {
+                const double bm = (double)b[m];
+                D[0][m] = fma(bm, dw[l][0], D[0][m]);
+                D[1][m] = fma(bm, dw[l][1], D[1][m]);
+                T[0][m] = fma(bm, w[l][0], T[0][m]);
+                T[1][m] = fma(bm, w[l][1], T[1][m]);
             }
         }
     }
@@ -601,10 +619,24 @@ __global__ void __launch_bounds__(NWARP * 32, 1) tdos_main(const MainParams p) {
 
                     const float4 es = sEs[t];
                     const uint2 cs = sCs[t];
-                    f2 wv[4], dw[4];
-                    corner_weights_x2(es.x, es.y, es.z, es.w, om, wv, dw);
                     const unsigned cc[4] = {cs.x & 0xffffu, cs.x >> 16, cs.y & 0xffffu, cs.y >> 16};
-                    acc.project(sW, cc, wv, dw);
+                    bool done = false;
+                    if constexpr (ACC64) {
+                        if (p.w64) {   // TDOS_ACC_FP64_ALL: the weights themselves in double precision
+                            double wa[4], da[4], wb[4], db[4];
+                            corner_weights_f64((double)es.x, (double)es.y, (double)es.z, (double)es.w, (double)om.x, wa, da);
+                            corner_weights_f64((double)es.x, (double)es.y, (double)es.z, (double)es.w, (double)om.y, wb, db);
+                            const double w2[4][2] = {{wa[0], wb[0]}, {wa[1], wb[1]}, {wa[2], wb[2]}, {wa[3], wb[3]}};
+                            const double d2[4][2] = {{da[0], db[0]}, {da[1], db[1]}, {da[2], db[2]}, {da[3], db[3]}};
+                            acc.project64(sW, cc, w2, d2);
+                            done = true;
+                        }
+                    }
+                    if (!done) {
+                        f2 wv[4], dw[4];
+                        corner_weights_x2(es.x, es.y, es.z, es.w, om, wv, dw);
+                        acc.project(sW, cc, wv, dw);
+                    }
                 }
             }
             if (worked) acc.flush(part, bin0, nE, norb, m0, vec4);

@@ -123,4 +123,56 @@ __device__ __forceinline__ void corner_weights_x2(float e1, float e2, float e3, 
     }
 }
 
+// The same weights in double precision for ONE energy (TDOS_ACC_FP64_ALL; "one can in principle switch to
+// double precision"): the algebra of corner_weights_x2 line by line -- bounded ratios, mirror image for Eq. 14,
+// derivative identities -- with true divisions instead of rcp.approx.  w[l] = w_l/V, dw[l] = (dw_l/dE)/V for the
+// sorted corners; all zero for an energy outside (e1, e4).  Eq. 15's constant is the caller's step histogram.
+__device__ __forceinline__ void corner_weights_f64(double e1, double e2, double e3, double e4, double E, double (&w)[4],
+                                                   double (&dw)[4]) {
+#pragma unroll
+    for (int l = 0; l < 4; l++) w[l] = dw[l] = 0.0;
+    if (!((E > e1) && (E < e4))) return;
+    const bool lo = E < e2, hi = E >= e3;
+    if (lo || hi) {
+        // Eq. 12 / Eq. 14: x = E - E1 (or E4 - E); far corners j: r_j = x/E_j1 (or x/E_4j) <= 1; C = r r' r''
+        const double x = lo ? E - e1 : e4 - E;
+        const double i1 = 1.0 / (lo ? e2 - e1 : e4 - e2);      // sorted corner 2
+        const double i2 = 1.0 / (lo ? e3 - e1 : e4 - e3);      // sorted corner 3
+        const double i3 = 1.0 / (e4 - e1);                     // the other outer corner
+        const double r1 = x * i1, r2 = x * i2, r3 = x * i3;
+        const double C = r1 * r2 * r3;                         // 12a / 14a
+        const double sg = lo ? 1.0 : -1.0;                     // Eq. 14: w - V = -C q
+        const double wF1 = sg * C * r1, wF2 = sg * C * r2, wF3 = sg * C * r3;      // 12e / 14c
+        const double dF1 = 4.0 * C * i1, dF2 = 4.0 * C * i2, dF3 = 4.0 * C * i3;   // 12f / 14d
+        const double wN = sg * C * (4.0 - (r1 + r2 + r3));                         // 12c / 14e
+        const double dN = 12.0 * r1 * r2 * i3 - (dF1 + dF2 + dF3);                 // 12d / 14f: sum_l dw_l = +-4 dC
+        const double one = lo ? 0.0 : 1.0;                     // Eq. 14c/e: w_j = V - C q_j
+        w[1] = wF1 + one;  dw[1] = dF1;
+        w[2] = wF2 + one;  dw[2] = dF2;
+        w[0] = (lo ? wN : wF3) + one;  dw[0] = lo ? dN : dF3;
+        w[3] = (lo ? wF3 : wN) + one;  dw[3] = lo ? dF3 : dN;
+        return;
+    }
+    // Eq. 13 (e2 <= E < e3; then e3 > e2, e3 > e1, e4 > e2, e4 > e1: no vanishing denominator)
+    const double i31 = 1.0 / (e3 - e1), i41 = 1.0 / (e4 - e1), i32 = 1.0 / (e3 - e2), i42 = 1.0 / (e4 - e2);
+    const double a = E - e1, b = E - e2, c = e3 - E, d = e4 - E;
+    const double A31 = a * i31, A41 = a * i41, B32 = b * i32, B42 = b * i42;
+    const double C31 = c * i31, C32 = c * i32, D41 = d * i41, D42 = d * i42;
+    const double C1 = A31 * A41;                                        // 13a
+    const double dC1 = 2.0 * A31 * i41;                                 // 13b
+    const double C2 = A41 * B32 * C31;                                  // 13c
+    const double dC2 = i41 * (C32 * (a + b) * i31 - A31 * B32);         // 13d
+    const double C3 = B32 * B42 * D41;                                  // 13e
+    const double dC3 = B32 * i41 * (2.0 * D42 - B42);                   // 13f
+    const double C12 = C1 + C2, C23 = C2 + C3, C123 = C12 + C3;
+    const double dC12 = dC1 + dC2, dC23 = dC2 + dC3, dC123 = dC12 + dC3;
+    const double P = C12 * C31, Q = C23 * C32, R = C123 * D41, S = C3 * D42;
+    const double dP = dC12 * C31 - C12 * i31, dQ = dC23 * C32 - C23 * i32;
+    const double dR = dC123 * D41 - C123 * i41, dS = dC3 * D42 - C3 * i42;
+    w[0] = C1 + P + R;                  dw[0] = dC1 + dP + dR;                    // 13g, 13h
+    w[1] = C123 + Q + S;                dw[1] = dC123 + dQ + dS;                  // 13i, 13j
+    w[2] = (C12 - P) + (C23 - Q);       dw[2] = (dC12 - dP) + (dC23 - dQ);        // 13k (G3), 13l (G4)
+    w[3] = (C123 - R) + (C3 - S);       dw[3] = (dC123 - dR) + (dC3 - dS);        // 13m, 13n
+}
+
 }  // namespace tdos

@@ -160,6 +160,7 @@ struct tdos_plan {
     int grid_rows = 0;
     bool adaptive = false;        // both kernels are enqueued; the device picks one per call (tdos_estimate)
     bool acc64 = false;           // tdos_plan_set_accumulation(TDOS_ACC_FP64): var64 runs, partials in fp64
+    bool w64 = false;             // TDOS_ACC_FP64_ALL: var64 also evaluates the corner weights in fp64
     Variant var64{};
     int grid64 = 0;
     double* partial64 = nullptr;  // [grid64] rows [nE_max + 3][3 * norb_alloc], allocated when the mode is first set
@@ -428,6 +429,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
     mp.counters = p->counters;
     mp.next_item = reinterpret_cast<unsigned int*>(p->counters + 3);
     mp.partial64 = p->partial64;
+    mp.w64 = (p->acc64 && p->w64) ? 1 : 0;
     const bool pair = p->adaptive && !p->acc64;   // both kernels enqueued, the device picks
     mp.est = pair ? p->counters + 4 : nullptr;
 
@@ -809,9 +811,9 @@ int tetra_dos_simple(const float* E, const float* W, int Nk, int nb, int norb, f
 }
 
 int tdos_plan_set_accumulation(tdos_plan* p, int mode) {
-    if (!p || (mode != TDOS_ACC_FP32 && mode != TDOS_ACC_FP64)) return TDOS_EINVAL;
+    if (!p || (mode != TDOS_ACC_FP32 && mode != TDOS_ACC_FP64 && mode != TDOS_ACC_FP64_ALL)) return TDOS_EINVAL;
     ON_DEVICE(p->device);
-    if (mode == TDOS_ACC_FP64 && !p->partial64) {
+    if (mode != TDOS_ACC_FP32 && !p->partial64) {
         p->var64 = variant64(pick_mb(p->norb));
         int bps = 0;
         cudaError_t e = cudaFuncSetAttribute((const void*)p->var64.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_optin);
@@ -827,7 +829,8 @@ int tdos_plan_set_accumulation(tdos_plan* p, int mode) {
         }
     }
     if (p->last_stream_valid) CK(cudaStreamSynchronize(p->last_stream));   // no call in flight changes its kernels
-    p->acc64 = (mode == TDOS_ACC_FP64);
+    p->acc64 = (mode != TDOS_ACC_FP32);
+    p->w64 = (mode == TDOS_ACC_FP64_ALL);
     return TDOS_OK;
 }
 

@@ -617,6 +617,64 @@ def test_fp64_accumulation_reaches_the_output_rounding_floor(cache_dir):
         print("%s fp64 accumulation dDOS %.2e dN %.2e (fp32: %.2e %.2e)" % (name, d64, n64, d32, n32))
 
 
+def _fp64_shares_vs_oracle(plan, E, W, nk, om, ref):
+    """tetra_dos_partial over the whole grid: the raw fp64 sums, turned into DOS and N in numpy fp64 exactly as
+    tetra_dos_finalize does (V * part[0]; V * (part[1] + inclusive prefix of part[2])) -- no fp32 rounding anywhere"""
+    import torch
+    dev = torch.device("cuda:0")
+    norb = 1 if W is None else W.shape[2]
+    dE, dOm = torch.from_numpy(E).to(dev), torch.from_numpy(om).to(dev)
+    dW = None if W is None else torch.from_numpy(W).to(dev)
+    part = torch.full((3, norb, len(om)), float("nan"), dtype=torch.float64, device=dev)
+    plan.tetra_dos_partial(dE, dW, dOm, 0, nk[2], part)
+    torch.cuda.synchronize()
+    P = part.cpu().numpy()
+    V = 1.0 / (24.0 * float(np.prod(nk)))
+    dos, nos = V * P[0], V * (P[1] + np.cumsum(P[2], axis=1))
+    ed = np.abs(dos - ref["dos"]).max() / ref["dos"].max()
+    pos = ref["nos"] > 0
+    en = (np.abs(nos - ref["nos"])[pos] / ref["nos"][pos]).max()
+    assert not nos[~pos].any()
+    return ed, en
+
+
+def test_all_fp64_mode_agrees_with_the_oracle_to_1e_12(cache_dir):
+    """PAPER.md:271 "one can in principle switch to double precision": with TDOS_ACC_FP64_ALL the corner weights are
+    double precision too, so the fp64 shares of tetra_dos_partial must agree with the fp64 oracle far below single
+    precision: 1e-12 on config 2 (DOS relative to its maximum, N relative wherever N > 0; measured 2e-15), against
+    2e-8 .. 4e-8 with fp32 weights.  Unstructured random energies (nearly degenerate tetrahedra): 1e-11 (measured 4e-15).  The fp32 outputs of tetra_dos in this
+    mode carry only their own rounding (1.5e-7)."""
+    cfg = wl.CONFIGS["cfg2"]
+    E, W, om, ref = _full_ref("cfg2", cache_dir)
+    with binding.Plan(cfg.nk, cfg.nb, cfg.norb, cfg.nE) as plan:
+        plan.set_accumulation(True)
+        d1, n1 = _fp64_shares_vs_oracle(plan, E, W, cfg.nk, om, ref)          # fp32 weights, fp64 sums
+        plan.set_accumulation(True, weights_fp64=True)
+        d2, n2 = _fp64_shares_vs_oracle(plan, E, W, cfg.nk, om, ref)
+        assert plan.last_counters()["kernel"] == 3
+        dos, nos = run_gpu(E, W, cfg.nk, om, plan=plan)
+        d3, n3, zero_ok = errors(ref, dos, nos)
+        plan.set_accumulation(False)
+        dos, nos = run_gpu(E, W, cfg.nk, om, plan=plan)
+        assert_parity(ref, dos, nos, "fp32 again")
+    print("cfg2 fp64 shares: fp32 weights dDOS %.2e dN %.2e; fp64 weights dDOS %.2e dN %.2e; fp32 outputs %.2e %.2e"
+          % (d1, n1, d2, n2, d3, n3))
+    assert d2 <= 1e-12 and n2 <= 1e-12, (d2, n2)
+    assert d1 > 10 * d2 and n1 > 10 * n2            # the mode does what it says: the fp32 weights were the floor
+    assert zero_ok and d3 <= 1.5e-7 and n3 <= 1.5e-7
+    for nk, nb, norb, nE in (((5, 3, 7), 3, 8, 333), ((6, 5, 4), 2, 3, 200), ((3, 4, 3), 1, 1, 64)):
+        E, W = wl.random_bands(nk, nb, norb, seed=41 + norb)
+        if norb == 1:
+            W = None
+        om = wl.omega_grid(-1.1, 1.2, nE)
+        ref = oracle.tetra_dos(E, W, nk, om)
+        with binding.Plan(nk, nb, norb, nE) as plan:
+            plan.set_accumulation(binding.TDOS_ACC_FP64_ALL)
+            d, n = _fp64_shares_vs_oracle(plan, E, W, nk, om, ref)
+        print("random %s fp64 weights dDOS %.2e dN %.2e" % (nk, d, n))
+        assert d <= 1e-11 and n <= 1e-11, (nk, d, n)
+
+
 @pytest.mark.parametrize("nk,nb,norb,nE", [((5, 3, 7), 3, 8, 333), ((6, 5, 4), 2, 3, 200), ((4, 4, 5), 2, 12, 150), ((3, 4, 3), 1, 1, 64)])
 def test_fp64_accumulation_on_unstructured_energies(nk, nb, norb, nE):
     """every orbital-block width, selection + total, W = NULL: north-star tolerances (the error left is that of the
