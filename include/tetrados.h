@@ -190,6 +190,16 @@ int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, 
                       int nE, int z_lo, int z_hi, double* part, void* cuda_stream);
 int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos,
                        void* cuda_stream);
+/*
+ * tetra_dos_partial for a GPU that holds only its own part of the grid ("each GPU holding its slab's
+ * k-planes plus one halo plane"): E and W hold the z_hi - z_lo + 1 k-planes z_lo, z_lo + 1, ..., z_hi of
+ * the grid in this order -- the last one is the halo, i.e. plane 0 again when z_hi == N3 -- and nothing else:
+ *     TDOS_AOS: E[kl][n], W[kl][n][m];   TDOS_SOA: E[n][kl], W[n][m][kl];   kl = ix + N1*(iy + N2*(iz - z_lo)),
+ * (N1*N2*(z_hi - z_lo + 1) k-points).  Requires z_lo < z_hi.  `part` and everything else as tetra_dos_partial; the two
+ * calls give the same share for the same slab.
+ */
+int tetra_dos_partial_slab(tdos_plan* p, const float* E, const float* W, int layout, const float* omega,
+                           int nE, int z_lo, int z_hi, double* part, void* cuda_stream);
 
 /*
  * Generic tetrahedron integration weights (Eq. 5-7, :58-71): for nW energies (device array, any order)

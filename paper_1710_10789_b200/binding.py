@@ -19,7 +19,7 @@ TDOS_STATIC_MAX_CELLS = 32768   # tetra_dos_static: norb * (nE rounded up to 4) 
 
 # every symbol include/tetrados.h declares
 SYMBOLS = ["tdos_version", "tdos_strerror", "tdos_last_cuda_error", "tdos_plan_create", "tdos_plan_destroy", "tdos_plan_set_accumulation",
-           "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_eigh", "tetra_weights", "tetra_dos_partial", "tetra_dos_finalize", "tetra_dos_simple", "tetra_dos_static", "tdos_plan_info",
+           "tetra_dos", "tetra_dos_complex", "tetra_dos_select", "tetra_eigh", "tetra_weights", "tetra_dos_partial", "tetra_dos_partial_slab", "tetra_dos_finalize", "tetra_dos_simple", "tetra_dos_static", "tdos_plan_info",
            "tdos_last_counters", "tdos_kernel_ms", "tdos_last_kernel_ms", "tdos_fp32_fma_probe"]
 
 _lib = None
@@ -58,6 +58,7 @@ def load():
     lib.tetra_eigh.argtypes = [vp, fp, fp, fp, vp]
     lib.tetra_weights.argtypes = [vp, fp, C.c_int, fp, C.c_int, fp, fp, vp]
     lib.tetra_dos_partial.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, C.c_int, C.c_int, vp, vp]
+    lib.tetra_dos_partial_slab.argtypes = [vp, fp, fp, C.c_int, fp, C.c_int, C.c_int, C.c_int, vp, vp]
     lib.tetra_dos_finalize.argtypes = [vp, vp, C.c_int, fp, fp, vp]
     lib.tetra_dos_simple.argtypes = [fp, fp, C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_int, fp, fp]
     lib.tetra_dos_static.argtypes = [ip, C.c_int, C.c_int, fp, fp, C.c_int, fp, C.c_int, fp, fp, vp]
@@ -160,6 +161,12 @@ class Plan:
         nE = int(omega.shape[0])
         _check(load().tetra_dos_partial(self._h, _ptr(E), _ptr(W), layout, _ptr(omega), nE, int(z_lo), int(z_hi),
                                         _ptr(part), _stream_ptr(stream, TDOS_DEVICE)), "tetra_dos_partial")
+
+    def tetra_dos_partial_slab(self, E, W, omega, z_lo: int, z_hi: int, part, layout: int = TDOS_AOS, stream=None):
+        """tetra_dos_partial_slab(): E, W hold only the k-planes z_lo .. z_hi (slab + halo plane) of the grid."""
+        nE = int(omega.shape[0])
+        _check(load().tetra_dos_partial_slab(self._h, _ptr(E), _ptr(W), layout, _ptr(omega), nE, int(z_lo), int(z_hi),
+                                             _ptr(part), _stream_ptr(stream, TDOS_DEVICE)), "tetra_dos_partial_slab")
 
     def tetra_dos_finalize(self, part, nE: int, dos, nos=None, stream=None):
         _check(load().tetra_dos_finalize(self._h, _ptr(part), int(nE), _ptr(dos), _ptr(nos),

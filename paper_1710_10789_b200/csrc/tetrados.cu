@@ -6,6 +6,7 @@
 
 #include <cuda_runtime.h>
 
+#include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -403,9 +404,12 @@ static int mark_end_of_call(tdos_plan* p, cudaStream_t st) {
 
 // enqueue the main kernel for the cube slab [z_lo, z_hi); `first` also clears the block partials and the
 // work counters (a call may cover the grid with several slab launches that accumulate into the same partials)
+// `nz_arr` > 0: E and W hold only the nz_arr = z_hi - z_lo + 1 planes z_lo .. z_hi of the grid (the last one is the halo,
+// plane z_hi mod N3), in that order (tetra_dos_partial_slab).  The kernels then run with base pointers moved back by z_lo
+// planes and with N3 = z_hi + 1, so that no z index they form wraps and plane z lands on local plane z - z_lo.
 static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
-                        int z_lo, int z_hi, bool first, cudaStream_t st) {
-    const long long nkt = (long long)p->nk[0] * p->nk[1] * p->nk[2];
+                        int z_lo, int z_hi, bool first, cudaStream_t st, int nz_arr = 0) {
+    const long long nkt = (long long)p->nk[0] * p->nk[1] * (nz_arr > 0 ? nz_arr : p->nk[2]);
     MainParams mp{};
     mp.E = E;
     mp.W = W;
@@ -418,6 +422,13 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         mp.sWk = 1; mp.sWn = (long long)p->norb * nkt; mp.sWm = nkt;
     }
     mp.N1 = p->nk[0]; mp.N2 = p->nk[1]; mp.N3 = p->nk[2];
+    if (nz_arr > 0) {
+        const long long k0 = (long long)p->nk[0] * p->nk[1] * z_lo;   // k-points in front of the slab
+        const long long wfl = (W != nullptr && p->cplx) ? 2 : 1;      // floats per weight element
+        mp.E = reinterpret_cast<const float*>(reinterpret_cast<uintptr_t>(E) - (uintptr_t)(k0 * mp.sEk) * sizeof(float));
+        if (W) mp.W = reinterpret_cast<const float*>(reinterpret_cast<uintptr_t>(W) - (uintptr_t)(k0 * mp.sWk * wfl) * sizeof(float));
+        mp.N3 = z_hi + 1;
+    }
     mp.nb = p->nb; mp.norb = p->k_norb; mp.nE = nE;
     mp.nsel = p->sel_n; mp.total = p->sel_total; mp.norb_in = p->norb;
     memcpy(mp.sel, p->sel, sizeof(mp.sel));
@@ -442,7 +453,7 @@ static int enqueue_main(tdos_plan* p, const float* E, const float* W, int layout
         p->last_launches = 0;
         if (pair && z_hi > z_lo) {   // sample the windows of this call's (first) slab: the device picks the kernel
             tdos::EstimateParams ep{};
-            ep.E = E; ep.omega = omega;
+            ep.E = mp.E; ep.omega = omega;
             ep.sEk = mp.sEk; ep.sEn = mp.sEn;
             ep.N1 = mp.N1; ep.N2 = mp.N2; ep.N3 = mp.N3; ep.nb = mp.nb; ep.nE = nE;
             ep.z_lo = z_lo; ep.z_hi = z_hi;
@@ -508,11 +519,11 @@ static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st
 
 // zero partials, main kernel over [z_lo, z_hi), merge into part_out; events around the main kernel
 static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
-                           int z_lo, int z_hi, double* part_out, cudaStream_t st) {
+                           int z_lo, int z_hi, double* part_out, cudaStream_t st, int nz_arr = 0) {
     int rc0 = order_after_last_call(p, st);
     if (rc0) return rc0;
     CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
-    int rc = enqueue_main(p, E, W, layout, omega, nE, z_lo, z_hi, true, st);
+    int rc = enqueue_main(p, E, W, layout, omega, nE, z_lo, z_hi, true, st, nz_arr);
     if (rc) return rc;
     CK(cudaEventRecord(p->ring[p->cur_slot][1], st));
     return enqueue_merge(p, nE, part_out, st);
@@ -535,6 +546,22 @@ int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, 
     reset_call_state(p);
     p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
     rc = enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream);
+    if (rc) return rc;
+    CK(cudaEventRecord(p->ring[p->cur_slot][2], (cudaStream_t)cuda_stream));
+    p->n_timed_calls++;
+    p->timed = true;
+    return mark_end_of_call(p, (cudaStream_t)cuda_stream);
+}
+
+int tetra_dos_partial_slab(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
+                           int z_lo, int z_hi, double* part, void* cuda_stream) {
+    int rc = check_common(p, E, W, layout, omega, nE);
+    if (rc) return rc;
+    if (!part || z_lo < 0 || z_hi > p->nk[2] || z_lo >= z_hi) return TDOS_EINVAL;   // an empty slab has no arrays to pass
+    ON_DEVICE(p->device);
+    reset_call_state(p);
+    p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
+    rc = enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream, z_hi - z_lo + 1);
     if (rc) return rc;
     CK(cudaEventRecord(p->ring[p->cur_slot][2], (cudaStream_t)cuda_stream));
     p->n_timed_calls++;

@@ -8,10 +8,15 @@ from . import sharding
 
 
 def sharded_step(plan, E, W, omega, nk3: int, rank: int, world: int, part, dos, nos, all_reduce, layout: int = 0,
-                 stream=None):
+                 stream=None, slab_local: bool = False):
     """One pass of the path on `world` ranks.  `part` is this rank's device tensor float64[3][norb][nE] (scratch),
-    `all_reduce(part)` must sum it over the ranks in place (and order itself after the work enqueued on `stream`)."""
+    `all_reduce(part)` must sum it over the ranks in place (and order itself after the work enqueued on `stream`).
+    slab_local: E and W hold only this rank's k-planes z_lo .. z_hi (sharding.planes_read: slab + halo plane) instead
+    of the whole grid."""
     z_lo, z_hi = sharding.z_slab(rank, world, nk3)
-    plan.tetra_dos_partial(E, W, omega, z_lo, z_hi, part, layout=layout, stream=stream)
+    if slab_local and z_hi > z_lo:
+        plan.tetra_dos_partial_slab(E, W, omega, z_lo, z_hi, part, layout=layout, stream=stream)
+    else:
+        plan.tetra_dos_partial(E, W, omega, z_lo, z_hi, part, layout=layout, stream=stream)
     all_reduce(part)
     plan.tetra_dos_finalize(part, int(omega.shape[0]), dos, nos, stream=stream)

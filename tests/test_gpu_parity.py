@@ -149,6 +149,24 @@ def test_partial_slabs_and_finalize():
         plan.tetra_dos_finalize(total, nE, dos, nos)
         torch.cuda.synchronize()
         assert_parity(ref, dos.cpu().numpy(), nos.cpu().numpy(), "slabs")
+        # the same with arrays that hold only a slab's planes plus its halo plane (tetra_dos_partial_slab): equal
+        # shares, AoS and SoA; the last slab's halo is plane 0
+        plane = nk[0] * nk[1]
+        for z_lo, z_hi in ((0, 4), (4, 5), (5, 9)):
+            zs = [z % nk[2] for z in range(z_lo, z_hi + 1)]
+            idx = np.concatenate([np.arange(z * plane, (z + 1) * plane) for z in zs])
+            El, Wl = np.ascontiguousarray(E[idx]), np.ascontiguousarray(W[idx])
+            want = torch.empty((3, norb, nE), dtype=torch.float64, device=dev)
+            plan.tetra_dos_partial(dE, dW, dOm, z_lo, z_hi, want)
+            for layout in (binding.TDOS_AOS, binding.TDOS_SOA):
+                Ex, Wx = (El, Wl) if layout == binding.TDOS_AOS else wl.to_soa(El, Wl)
+                got = torch.full((3, norb, nE), float("nan"), dtype=torch.float64, device=dev)
+                plan.tetra_dos_partial_slab(torch.from_numpy(Ex).to(dev), torch.from_numpy(Wx).to(dev), dOm, z_lo, z_hi, got,
+                                            layout=layout)
+                torch.cuda.synchronize()
+                assert torch.allclose(got, want, rtol=1e-5, atol=1e-9 * float(want.abs().max())), (z_lo, z_hi, layout)
+        with pytest.raises(binding.TdosError):
+            plan.tetra_dos_partial_slab(dE, dW, dOm, 4, 4, part)          # an empty slab
         # one slab against the oracle's share of the same cubes
         part = torch.empty((3, norb, nE), dtype=torch.float64, device=dev)
         plan.tetra_dos_partial(dE, dW, dOm, 4, 5, part)

@@ -47,11 +47,23 @@ def _worker(rank, world, port, out):
             dist.all_reduce(h)
             t.copy_(h)
 
+        # what SURVEY.md 8(e) describes: this rank's k-planes only (its slab plus the halo plane), nothing else on the device
+        from paper_1710_10789_b200 import sharding
+        plane = nk[0] * nk[1]
+        idx = np.concatenate([np.arange(z * plane, (z + 1) * plane) for z in sharding.planes_read(rank, world, nk[2])])
+        lE, lW = torch.from_numpy(np.ascontiguousarray(E[idx])).to(dev), torch.from_numpy(np.ascontiguousarray(W[idx])).to(dev)
         with binding.Plan(nk, nb, norb, nE) as plan:
             for _ in range(2):       # twice on one plan: the shares do not accumulate across calls
                 multigpu.sharded_step(plan, dE, dW, dOm, nk[2], rank, world, part, dos, nos, all_reduce)
                 torch.cuda.synchronize()
+            full = (dos.clone(), nos.clone())
+            dos.fill_(float("nan"))
+            nos.fill_(float("nan"))
+            multigpu.sharded_step(plan, lE, lW, dOm, nk[2], rank, world, part, dos, nos, all_reduce, slab_local=True)
+            torch.cuda.synchronize()
             cnt = plan.last_counters()
+            assert torch.allclose(dos, full[0], rtol=1e-5, atol=1e-7 * float(full[0].max()))
+            assert torch.allclose(nos, full[1], rtol=1e-5, atol=1e-7 * float(full[1].max()))
         c = torch.tensor([cnt["n_tb"], cnt["n_eval"]])
         dist.all_reduce(c)
         ref = oracle.tetra_dos(E, W, nk, om)
