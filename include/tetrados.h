@@ -49,7 +49,11 @@
  * scratch (block partials, staging buffers, its side stream), shared by all its calls: calls are executed one after the
  * other even when issued on different streams (a call on another stream than the previous one first waits, on the
  * device, for that one's end).  A plan must not be used from two host threads at the same time.  Inputs are never
- * written.  Every entry point runs on the plan's device and restores the caller's current device before it returns.
+ * written.  CUDA graphs: a TDOS_DEVICE call (tetra_dos, _select, _complex, _partial, _partial_slab, _finalize) whose
+ * stream is being captured is recorded into the graph -- memsets and kernels only; the plan's ordering and timing
+ * events are left out, so tdos_kernel_ms does not see it and a replay is ordered against other calls on the plan only
+ * by what the caller orders: do not run a replay concurrently with another call on the same plan.  The call captured
+ * first on a plan should not be the plan's very first call (the first call of a kernel loads it).  Every entry point runs on the plan's device and restores the caller's current device before it returns.
  *
  * Errors: every function returns 0 (TDOS_OK) or a negative code; nothing throws, exits or prints.
  * On error the outputs are untouched (host mode) / unspecified only if TDOS_ECUDA occurred mid-flight.

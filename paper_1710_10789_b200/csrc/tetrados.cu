@@ -202,6 +202,9 @@ struct tdos_plan {
     cudaStream_t last_stream = nullptr;
     bool last_stream_valid = false;
     bool timed = false;
+    // the device-mode call being enqueued goes into a stream capture (CUDA graph): the plan's own events are left out
+    // of it -- an event recorded inside a capture cannot be waited on or timed outside, and the other way round
+    bool cap = false;
     long long last_items = 0, last_launches = 0;
 };
 
@@ -393,13 +396,37 @@ static int rows_per_block(int nE) { return (nE + 3) & ~3; }
 // The plan's scratch (partials, counters, merge buffer) is shared by all calls: a call on another stream than the
 // previous one waits for that one's end.
 static int order_after_last_call(tdos_plan* p, cudaStream_t st) {
+    if (p->cap) return TDOS_OK;   // a captured call is ordered by the graph's own dependencies (include/tetrados.h)
     if (p->done_valid && !(p->last_stream_valid && p->last_stream == st)) CK(cudaStreamWaitEvent(st, p->done_ev, 0));
     return TDOS_OK;
 }
 static int mark_end_of_call(tdos_plan* p, cudaStream_t st) {
+    if (p->cap) return TDOS_OK;
     CK(cudaEventRecord(p->done_ev, st));
     p->done_valid = true;
     return TDOS_OK;
+}
+// is `st` being captured?  (sets p->cap for the helpers of this call)
+static int note_capture(tdos_plan* p, cudaStream_t st) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    CK(cudaStreamIsCapturing(st, &cs));
+    p->cap = (cs != cudaStreamCaptureStatusNone);
+    return TDOS_OK;
+}
+// timing events of the ring: not recorded into a capture
+static cudaError_t ring_record(tdos_plan* p, int which, cudaStream_t st) {
+    return p->cap ? cudaSuccess : cudaEventRecord(p->ring[p->cur_slot][which], st);
+}
+// bookkeeping at the end of a device-mode call
+static int end_of_device_call(tdos_plan* p, cudaStream_t st) {
+    CK(ring_record(p, 2, st));
+    if (!p->cap) {
+        p->n_timed_calls++;
+        p->timed = true;
+    }
+    const int rc = mark_end_of_call(p, st);
+    p->cap = false;
+    return rc;
 }
 
 // enqueue the main kernel for the cube slab [z_lo, z_hi); `first` also clears the block partials and the
@@ -520,12 +547,14 @@ static int enqueue_merge(tdos_plan* p, int nE, double* part_out, cudaStream_t st
 // zero partials, main kernel over [z_lo, z_hi), merge into part_out; events around the main kernel
 static int enqueue_partial(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
                            int z_lo, int z_hi, double* part_out, cudaStream_t st, int nz_arr = 0) {
-    int rc0 = order_after_last_call(p, st);
+    int rc0 = note_capture(p, st);
     if (rc0) return rc0;
-    CK(cudaEventRecord(p->ring[p->cur_slot][0], st));
+    rc0 = order_after_last_call(p, st);
+    if (rc0) return rc0;
+    CK(ring_record(p, 0, st));
     int rc = enqueue_main(p, E, W, layout, omega, nE, z_lo, z_hi, true, st, nz_arr);
     if (rc) return rc;
-    CK(cudaEventRecord(p->ring[p->cur_slot][1], st));
+    CK(ring_record(p, 1, st));
     return enqueue_merge(p, nE, part_out, st);
 }
 
@@ -547,10 +576,7 @@ int tetra_dos_partial(tdos_plan* p, const float* E, const float* W, int layout, 
     p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
     rc = enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream);
     if (rc) return rc;
-    CK(cudaEventRecord(p->ring[p->cur_slot][2], (cudaStream_t)cuda_stream));
-    p->n_timed_calls++;
-    p->timed = true;
-    return mark_end_of_call(p, (cudaStream_t)cuda_stream);
+    return end_of_device_call(p, (cudaStream_t)cuda_stream);
 }
 
 int tetra_dos_partial_slab(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
@@ -563,10 +589,7 @@ int tetra_dos_partial_slab(tdos_plan* p, const float* E, const float* W, int lay
     p->cur_slot = (int)(p->n_timed_calls % tdos_plan::kRing);
     rc = enqueue_partial(p, E, W, layout, omega, nE, z_lo, z_hi, part, (cudaStream_t)cuda_stream, z_hi - z_lo + 1);
     if (rc) return rc;
-    CK(cudaEventRecord(p->ring[p->cur_slot][2], (cudaStream_t)cuda_stream));
-    p->n_timed_calls++;
-    p->timed = true;
-    return mark_end_of_call(p, (cudaStream_t)cuda_stream);
+    return end_of_device_call(p, (cudaStream_t)cuda_stream);
 }
 
 int tetra_dos_finalize(tdos_plan* p, const double* part, int nE, float* dos, float* nos, void* cuda_stream) {
@@ -583,10 +606,7 @@ static int run_device(tdos_plan* p, const float* E, const float* W, int layout, 
     if (rc) return rc;
     rc = enqueue_finalize(p, p->part64, nE, dos, nos, st);
     if (rc) return rc;
-    CK(cudaEventRecord(p->ring[p->cur_slot][2], st));
-    p->n_timed_calls++;
-    p->timed = true;
-    return mark_end_of_call(p, st);
+    return end_of_device_call(p, st);
 }
 
 static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layout, const float* omega, int nE,
@@ -673,6 +693,7 @@ static int tetra_dos_impl(tdos_plan* p, const float* E, const float* W, int layo
     // also plane 0), so the cubes of slab s -- which read planes z_s .. z_{s+1}, the last one wrapping to
     // plane 0 -- need copies 0..s only.
     cudaStream_t st = p->main, cp = p->side;
+    p->cap = false;   // host mode runs on the plan's own streams, which are never captured
     rc = order_after_last_call(p, st);
     if (rc) return rc;
     const int N3 = p->nk[2];

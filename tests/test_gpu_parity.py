@@ -497,6 +497,53 @@ def test_back_to_back_calls_on_two_streams():
         assert_parity(r, outs[i][0].cpu().numpy(), outs[i][1].cpu().numpy(), "two streams, call %d" % i)
 
 
+def test_device_mode_call_can_be_captured_in_a_cuda_graph():
+    """A TDOS_DEVICE call only enqueues work (memsets, kernels, event records) on the caller's stream, so it can be
+    recorded into a CUDA graph and replayed: PAPER.md:289's best case (inputs already on the GPU) inside a host loop
+    that re-launches one graph per iteration.  Captured on a side stream (a) right after a call on the same stream and
+    (b) right after a call on ANOTHER stream (the plan then makes the capturing stream wait for that call's end-of-call
+    event); every replay sees new band energies written in place and must match the oracle.  The timing diagnostics
+    (tdos_kernel_ms) are not available for captured calls; the counters are."""
+    import torch
+    dev = torch.device("cuda:0")
+    nk, nb, norb, nE = (12, 10, 8), 8, 8, 600
+    E, W = wl.tb8_bands(nk, threads=1)
+    om = wl.omega_grid(-6.0, 4.0, nE)
+    shifts = (0.0, 0.11, -0.23)
+    refs = [oracle.tetra_dos(E + np.float32(sh), W, nk, om, nthreads=_threads()) for sh in shifts]
+    dW, dOm = torch.from_numpy(W).to(dev), torch.from_numpy(om).to(dev)
+    for other_stream_first in (False, True):
+        dE = torch.from_numpy(E).to(dev)
+        dos = torch.zeros((norb, nE), device=dev)
+        nos = torch.zeros((norb, nE), device=dev)
+        side = torch.cuda.Stream()
+        with binding.Plan(nk, nb, norb, nE) as plan:
+            with torch.cuda.stream(side):
+                plan.tetra_dos(dE, dW, dOm, dos, nos, stream=side)          # warm-up on the capture stream
+            torch.cuda.synchronize()
+            if other_stream_first:
+                plan.tetra_dos(dE, dW, dOm, dos, nos)                        # last call before the capture: current stream
+                torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                plan.tetra_dos(dE, dW, dOm, dos, nos, stream=torch.cuda.current_stream())
+            for sh, ref in zip(shifts, refs):
+                dE.copy_(torch.from_numpy(E + np.float32(sh)))
+                dos.fill_(float("nan"))
+                nos.fill_(float("nan"))
+                torch.cuda.synchronize()
+                g.replay()
+                torch.cuda.synchronize()
+                assert_parity(ref, dos.cpu().numpy(), nos.cpu().numpy(), "graph replay, shift %g" % sh)
+            assert plan.last_counters()["n_eval"] == refs[-1]["n_eval"]
+            # an ordinary call on the same plan afterwards still works
+            dE.copy_(torch.from_numpy(E))
+            plan.tetra_dos(dE, dW, dOm, dos, nos)
+            torch.cuda.synchronize()
+            assert_parity(refs[0], dos.cpu().numpy(), nos.cpu().numpy(), "call after the graph")
+            del g
+
+
 @pytest.mark.parametrize("host", [False, True])
 def test_orbital_selection_plus_total_paper_shape(cache_dir, host):
     """five selected orbitals of the 8-orbital model and the total DOS on the
