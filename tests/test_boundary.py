@@ -36,7 +36,7 @@ def test_header_symbols_are_exported(binding):
 
 def test_version_and_strerror(binding):
     assert binding.tdos_version() >= 100
-    for code in (0, -1, -2, -3, -4, -99):
+    for code in (0, -1, -2, -3, -4, -5, -99):
         assert isinstance(binding.tdos_strerror(code), str) and binding.tdos_strerror(code)
 
 
