@@ -102,7 +102,7 @@ __device__ __forceinline__ void jacobi_round(double (&hr)[8], double (&hi)[8], d
     }
 }
 
-__global__ void __launch_bounds__(128) tdos_eigh8(const EighParams P) {
+__global__ void __launch_bounds__(128, 4) tdos_eigh8(const EighParams P) {
     const int lane = threadIdx.x & 31, r = lane & 7, base = lane & ~7;
     const long long mat = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 3;
     const bool live = mat < P.nmat;
