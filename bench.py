@@ -355,7 +355,7 @@ def workload_config(cfg, n_gpus: int, layout: str = "aos") -> dict:
 # `ncu --set full` capture (profiles/, named there); None until a capture of that config exists.
 # The number is a constant from that file, NOT measured in this run: `roofline.traffic_source` names the file.
 NCU_TRAFFIC_BYTES = {("cfg4", 3): (1.394956e9 + 280.968e6, "profiles/r01_v3_regions_cfg4.md"),
-                     ("cfg4", 5): (739.961e6 + 79.961e6, "profiles/r02_v5_main_cfg4.md"),
+                     ("cfg4", 5): (739.806e6 + 81.059e6, "profiles/r03_cfg4.md"),
                      ("cfg5", 3): (2.604243e9 + 120.008e6, "profiles/r02_v3_main_cfg5.md")}
 
 
